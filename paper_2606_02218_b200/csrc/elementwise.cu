@@ -1,0 +1,118 @@
+// elementwise.cu -- embedding gather, RoPE + bf16 KV append, row gathers (steps a5, a6).
+#include "common.cuh"
+#include "kernels.cuh"
+
+namespace sagc {
+
+// x[row][:] = embed[tok[row]][:] widened to fp32.  One CTA per row, 8 elements per thread-iteration.
+__global__ void __launch_bounds__(128) k_embed(const bf16_t* __restrict__ embed, const int* __restrict__ tok,
+                                               const int* m_dev, int m_max, int d, float* __restrict__ x) {
+    pdl_wait();
+    pdl_launch();
+    const int M = m_dev ? min(*m_dev, m_max) : m_max;
+    const int row = blockIdx.x;
+    if (row >= M) return;
+    const bf16_t* src = embed + (size_t)tok[row] * d;
+    float* dst = x + (size_t)row * d;
+    for (int k = threadIdx.x * 8; k < d; k += blockDim.x * 8) {
+        uint4 w = *reinterpret_cast<const uint4*>(src + k);
+        float4 a = make_float4(bf16lo_to_f32(w.x), bf16hi_to_f32(w.x), bf16lo_to_f32(w.y), bf16hi_to_f32(w.y));
+        float4 b = make_float4(bf16lo_to_f32(w.z), bf16hi_to_f32(w.z), bf16lo_to_f32(w.w), bf16hi_to_f32(w.w));
+        *reinterpret_cast<float4*>(dst + k) = a;
+        *reinterpret_cast<float4*>(dst + k + 4) = b;
+    }
+}
+
+int launch_embed(const bf16_t* embed, const int* tok, const int* m_dev, int m_max, int d, float* x,
+                 cudaStream_t st) {
+    if (m_max <= 0) return 0;
+    k_embed<<<m_max, 128, 0, st>>>(embed, tok, m_dev, m_max, d, x);
+    return 1;
+}
+
+// RoPE (rotate-half: pairs (i, i+hd/2), table cos/sin from fp64 angles) on the q and k heads of
+// one activation row; q is rotated in place (fp32); k (rotated) and v are rounded to bf16 (RNE)
+// and written to slot pos%page of page page_table[sid][pos/page] -- the ONLY rounding point of
+// the forward pass (reading C1).  grid = (rows, Hq+2*Hkv heads), block = hd/2 threads.
+__global__ void k_rope_append(RopeArgs a) {
+    pdl_wait();
+    pdl_launch();
+    const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
+    const int row = blockIdx.x;
+    if (row >= M) return;
+    const int head = blockIdx.y;
+    const int half = a.hd >> 1;
+    const int i = threadIdx.x;
+    if (i >= half) return;
+    const int pos = a.row_pos[row];
+    const int ld = (a.Hq + 2 * a.Hkv) * a.hd;
+    float* hp = a.qkv + (size_t)row * ld + (size_t)head * a.hd;
+    float x0 = hp[i], x1 = hp[i + half];
+    if (head < a.Hq + a.Hkv) {
+        const float2 cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)pos * half + i) * 2);
+        float r0 = x0 * cs.x - x1 * cs.y;
+        float r1 = x1 * cs.x + x0 * cs.y;
+        x0 = r0; x1 = r1;
+    }
+    if (head < a.Hq) {
+        hp[i] = x0; hp[i + half] = x1;
+        return;
+    }
+    const int sid = a.row_sid[row];
+    const int pg = a.page_table[(size_t)sid * a.max_blocks + pos / a.page];
+    if (pg < 0) return;   // unmapped (only after a pool-exhaustion error)
+    const int isv = head >= a.Hq + a.Hkv;
+    const int kvh = head - a.Hq - (isv ? a.Hkv : 0);
+    bf16_t* dst = a.kv_layer + (((size_t)pg * 2 + isv) * a.Hkv + kvh) * (size_t)a.page * a.hd +
+                  (size_t)(pos % a.page) * a.hd;
+    dst[i] = (bf16_t)f32_to_bf16_bits(x0);
+    dst[i + half] = (bf16_t)f32_to_bf16_bits(x1);
+}
+
+int launch_rope_append(const RopeArgs& a, cudaStream_t st) {
+    if (a.m_max <= 0) return 0;
+    dim3 grid(a.m_max, a.Hq + 2 * a.Hkv);
+    k_rope_append<<<grid, a.hd / 2, 0, st>>>(a);
+    return 1;
+}
+
+// out[i][:] = x[row_idx[i]][:]
+__global__ void k_gather_rows(const float* __restrict__ x, const int* __restrict__ row_idx, int d,
+                              float* __restrict__ out) {
+    const float* src = x + (size_t)row_idx[blockIdx.x] * d;
+    float* dst = out + (size_t)blockIdx.x * d;
+    for (int k = threadIdx.x; k < d; k += blockDim.x) dst[k] = src[k];
+}
+int launch_gather_rows(const float* x, const int* row_idx, int n, int d, float* out, cudaStream_t st) {
+    if (n <= 0) return 0;
+    k_gather_rows<<<n, 256, 0, st>>>(x, row_idx, d, out);
+    return 1;
+}
+
+// Prefill row descriptors: row r of prompt p at offset j: sid = p*G (the group's first
+// completion owns the prefill writes), pos = j, ctx = j + 1, tok = prompt token.
+__global__ void k_prefill_rows(const int* __restrict__ prompt_tokens, const int* __restrict__ offs, int n_prompts,
+                               int G, int total, int* row_sid, int* row_pos, int* row_ctx, int* row_tok) {
+    int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= total) return;
+    int lo = 0, hi = n_prompts;          // largest p with offs[p] <= r
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (offs[mid] <= r) lo = mid; else hi = mid;
+    }
+    int j = r - offs[lo];
+    row_sid[r] = lo * G;
+    row_pos[r] = j;
+    row_ctx[r] = j + 1;
+    row_tok[r] = prompt_tokens[r];
+}
+int launch_prefill_rows(const int* prompt_tokens, const int* prompt_offsets_dev, int n_prompts, int G,
+                        int total_rows, int* row_sid, int* row_pos, int* row_ctx, int* row_tok,
+                        cudaStream_t st) {
+    if (total_rows <= 0) return 0;
+    k_prefill_rows<<<(total_rows + 255) / 256, 256, 0, st>>>(prompt_tokens, prompt_offsets_dev, n_prompts, G,
+                                                             total_rows, row_sid, row_pos, row_ctx, row_tok);
+    return 1;
+}
+
+}  // namespace sagc

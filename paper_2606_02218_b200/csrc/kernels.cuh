@@ -1,0 +1,122 @@
+// kernels.cuh -- launcher prototypes of the sm_100a kernels (internal; the public boundary is
+// include/sagc.h).  Every launcher enqueues on `st` and returns the number of kernels it launched.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace sagc {
+
+typedef uint16_t bf16_t;   // raw bf16 bit pattern
+
+enum { EPI_STORE = 0, EPI_RESID = 1, EPI_SWIGLU = 2 };
+enum { LIN_MMA = 0, LIN_GEMV = 1 };
+
+// Y[M][N] = epi( rms?(X)[M][K] . W[N][K]^T ).  Steps a6, a8-a11 of DESIGN.md.
+struct LinearArgs {
+    const bf16_t* W[3];     // up to three row segments (q,k,v) -- or {gate, up} for EPI_SWIGLU
+    int rows[3];            // rows per segment (EPI_SWIGLU: rows[0] == rows[1] == N)
+    const float* X;         // [M][K] fp32 activations
+    const bf16_t* norm_w;   // if non-null: fused RMSNorm, X <- X * norm_w * rsqrt(mean(X^2)+eps)
+    float eps;
+    float* Y;               // [M][ldy]
+    const float* R;         // EPI_RESID: Y = R + acc (R may alias Y)
+    int ldy;
+    int K, N;
+    const int* m_dev;       // device pointer to the live row count, or null
+    int m_max;              // grid is sized for this many rows (>= *m_dev)
+    int epi;
+    int kind;               // LIN_MMA | LIN_GEMV
+    bool pdl;               // launch with programmatic stream serialization
+};
+int launch_linear(const LinearArgs& a, cudaStream_t st);
+
+// x[row][d] = embed[tok[row]][d]  (fp32 residual stream).  Step a5.
+int launch_embed(const bf16_t* embed, const int* tok, const int* m_dev, int m_max, int d, float* x,
+                 cudaStream_t st);
+
+// RoPE on q and k heads, K/V rounded to bf16 (RNE) and appended to the sequence's page.  Step a6.
+struct RopeArgs {
+    float* qkv;             // [M][(Hq+2Hkv)*hd] fp32, q part rotated in place
+    const int* row_sid;     // [M] page-table row of each activation row
+    const int* row_pos;     // [M] position of each row
+    const int* m_dev; int m_max;
+    const float* rope_cs;   // [max_ctx][hd/2][2] (cos, sin) fp32, angles evaluated in fp64
+    bf16_t* kv_layer;       // this layer's pool: [n_pages][2][Hkv][page][hd]
+    const int* page_table;  // [max_seqs][max_blocks]
+    int max_blocks, page, Hq, Hkv, hd;
+};
+int launch_rope_append(const RopeArgs& a, cudaStream_t st);
+
+// Paged GQA attention over ragged contexts with split-K + in-kernel LSE merge.  Step a7.
+struct AttnArgs {
+    const float* q;         // [M][ldq] (first Hq*hd columns are the rotated queries)
+    int ldq;
+    const bf16_t* kv_layer; // [n_pages][2][Hkv][page][hd]
+    const int* page_table; int max_blocks;
+    const int* row_sid;     // [M]
+    const int* row_ctx;     // [M] number of cached positions attended (incl. the current one)
+    const int* m_dev; int m_max;
+    int Hq, Hkv, hd, page;
+    int n_splits;           // grid.z; every split covers ceil(ctx/n_splits) rounded up to a page
+    float* part_o;          // [M][Hq][n_splits][hd] scratch
+    float* part_ml;         // [M][Hq][n_splits][2]  (max, sum)
+    int* counters;          // [M*Hkv] arrival counters (zero on entry, reset on exit)
+    float* out;             // [M][Hq*hd]
+};
+int launch_attention(const AttnArgs& a, cudaStream_t st);
+
+// Sampler over fp32 logits.  Step a3 / a12.
+struct SampleArgs {
+    const float* logits;    // [M][V]
+    int V;
+    const int* row_sid;     // [M] completion id keyed into Philox (never the batch slot)
+    const int* step_dev;    // [1] 1-based generated-token index t
+    const int* m_dev; int m_max;
+    const uint32_t* params; // device [4] = mode, temperature (float bits), Philox key lo, key hi
+    int row_div;            // logits row of activation row i is i / row_div (first token: G)
+    int* out_tok;           // [M]
+};
+int launch_sample(const SampleArgs& a, cudaStream_t st);
+int launch_philox_debug(uint64_t seed, int sid, int t, int v0, int n, uint32_t* out, cudaStream_t st);
+
+// Segmented per-group statistics.  Step a14.
+int launch_group_advantage(const float* rewards, const int* offs, int n_groups, int mode, int ddof,
+                           float eps, float* adv, uint8_t* keep, cudaStream_t st);
+int launch_length_stats(const int* lengths, const int* offs, int n_groups, int* stats, float* ratio,
+                        cudaStream_t st);
+
+// Paging / retirement state machine (steps a1, a4, a13).  All arrays live on the device.
+struct PageState {
+    int* free_stack; int* n_free; int* refcnt; int* page_table; int* n_blocks; int* n_shared;
+    int* live; int* n_live; int* pos; int* ctx; int* tok; int* step; int* err; int* peak_used;
+    int* alloc_log; int* n_alloc; int* retire_log; int* n_retire; int log_cap_alloc, log_cap_retire;
+    int n_pages, max_blocks, page, max_seqs;
+};
+struct RolloutDev {
+    const int* prompt_len;      // [n_prompts]
+    const int* forced_len;      // [nseq] or null
+    const int* forced_tok;      // [nseq][max_new] or null
+    int* out_tokens;            // [nseq][max_new]
+    int* out_lengths;           // [nseq]
+    int n_prompts, G, nseq, max_new, stop_token, log;
+};
+int launch_pool_reset(const PageState& ps, const RolloutDev& rd, cudaStream_t st);
+int launch_prefill_alloc(const PageState& ps, const RolloutDev& rd, cudaStream_t st);
+// End of step t (retire / free / compact) + start of step t+1 (page alloc, pos/ctx/tok).
+// `sampled` holds the sampler's token for each live slot; first_step: slots are sids (t = 1).
+int launch_advance(const PageState& ps, const RolloutDev& rd, const int* sampled, int structure_only,
+                   cudaStream_t st);
+// Prefill helpers: row_sid/row_pos/row_ctx/tok for every prompt token, and the copy of a partial
+// last prompt block into the first private page of completions g >= 1.
+int launch_prefill_rows(const int* prompt_tokens, const int* prompt_offsets_dev, int n_prompts, int G,
+                        int total_rows, int* row_sid, int* row_pos, int* row_ctx, int* row_tok,
+                        cudaStream_t st);
+int launch_copy_partial_block(const PageState& ps, const RolloutDev& rd, bf16_t* kv_pool,
+                              size_t layer_stride, int n_layers, int page_elems, cudaStream_t st);
+// Gather the last prompt row of each prompt's logits source: xlast[p] = x[offsets[p+1]-1].
+int launch_gather_rows(const float* x, const int* row_idx, int n, int d, float* out, cudaStream_t st);
+// Copy the logits row of every (sid, t) dump request whose t equals the current step.
+int launch_dump_logits(const int* dump_sid_t, int n_dump, const int* step_dev, const int* live, const int* n_live,
+                       int row_div, const float* logits, int V, float* out, cudaStream_t st);
+
+}  // namespace sagc

@@ -1,0 +1,749 @@
+// runtime.cu -- host side of the C ABI (include/sagc.h): model handle, KV pool, step loop,
+// CUDA graphs, phase accounting.  No CPU fallback: every compute entry point needs a device.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <map>
+#include <string>
+#include <vector>
+
+#include "../../include/sagc.h"
+#include "common.cuh"
+#include "kernels.cuh"
+
+using namespace sagc;
+
+static thread_local char g_err[512] = "";
+static int set_err(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+extern "C" const char* sagc_last_error(void) { return g_err; }
+extern "C" const char* sagc_version(void) { return "sagc-rollout 0.1 (sm_100a)"; }
+
+#define CU(x)                                                                                   \
+    do {                                                                                        \
+        cudaError_t e_ = (x);                                                                   \
+        if (e_ != cudaSuccess)                                                                  \
+            return set_err(e_ == cudaErrorMemoryAllocation ? SAGC_ENOMEM : SAGC_ECUDA, "%s: %s (%s:%d)", #x, \
+                           cudaGetErrorString(e_), __FILE__, __LINE__);                         \
+    } while (0)
+
+static int env_int(const char* name, int dflt) {
+    const char* s = getenv(name);
+    return s ? atoi(s) : dflt;
+}
+
+struct GraphKey {
+    int m_max, n_splits, kind, dump;
+    bool operator<(const GraphKey& o) const {
+        if (m_max != o.m_max) return m_max < o.m_max;
+        if (n_splits != o.n_splits) return n_splits < o.n_splits;
+        if (kind != o.kind) return kind < o.kind;
+        return dump < o.dump;
+    }
+};
+struct GraphVal { cudaGraphExec_t exec; int n_kernels; };
+
+struct sagc_model {
+    sagc_model_config cfg;
+    std::vector<const bf16_t*> wq, wk, wv, wo, wg, wu, wd, norm1, norm2;
+    const bf16_t *embed, *lm_head, *final_norm;
+    int Nqkv, max_blocks, max_rows, max_splits;
+    size_t page_elems, layer_stride;          // bf16 elements per (layer, page) and per layer
+    std::vector<void*> allocs;                 // everything cudaMalloc'ed by the handle
+    bf16_t* kv_pool;
+    float* rope_cs;
+    PageState ps;
+    // scratch activations
+    float *x, *qkv, *att, *act, *logits, *xlast, *part_o, *part_ml;
+    int *counters, *sampled, *row_sid, *row_pos, *row_ctx, *row_tok, *last_idx, *prompt_len_d, *offs_d;
+    int row_cap;
+    // per-call device buffers (grown on demand)
+    int *tok_buf, *len_buf, *forced_len_d, *dump_list_d, *prompt_tok_d;
+    size_t tok_cap, forced_cap, dump_cap, prompt_cap;
+    uint32_t* sample_params_d;                 // [mode, temperature bits, key lo, key hi]
+    // graph cache, valid for one rollout signature
+    std::map<GraphKey, GraphVal> graphs;
+    std::string signature;
+    int last_nseq, last_max_blocks;
+    bool use_pdl;
+    int gemv_max;
+};
+
+template <typename T>
+static int dev_alloc(sagc_model* m, T** p, size_t n) {
+    void* q = nullptr;
+    cudaError_t e = cudaMalloc(&q, n * sizeof(T) + 256);
+    if (e != cudaSuccess) return set_err(SAGC_ENOMEM, "cudaMalloc(%zu bytes): %s", n * sizeof(T), cudaGetErrorString(e));
+    m->allocs.push_back(q);
+    *p = reinterpret_cast<T*>(q);
+    return SAGC_OK;
+}
+#define DA(ptr, n)                                         \
+    do {                                                   \
+        int rc_ = dev_alloc(m, &(ptr), (size_t)(n));       \
+        if (rc_ != SAGC_OK) { sagc_model_destroy(m); return rc_; } \
+    } while (0)
+
+static void clear_graphs(sagc_model* m) {
+    for (auto& kv : m->graphs) cudaGraphExecDestroy(kv.second.exec);
+    m->graphs.clear();
+}
+
+extern "C" void sagc_model_destroy(sagc_model* m) {
+    if (!m) return;
+    clear_graphs(m);
+    for (void* p : m->allocs) cudaFree(p);
+    delete m;
+}
+
+static const int PREFILL_ROWS = 2048;
+
+extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weights* w, sagc_model** out) {
+    if (!cfg || !w || !out) return set_err(SAGC_EINVAL, "null argument");
+    const sagc_model_config& c = *cfg;
+    if (c.head_dim != 32 && c.head_dim != 64 && c.head_dim != 128) return set_err(SAGC_EINVAL, "head_dim must be 32, 64 or 128");
+    if (c.n_kv_heads <= 0 || c.n_q_heads % c.n_kv_heads != 0 || c.n_q_heads / c.n_kv_heads > 8)
+        return set_err(SAGC_EINVAL, "n_q_heads / n_kv_heads must be an integer <= 8");
+    if (c.d_model % 32 || c.d_ff % 32 || c.vocab % 16 || (c.n_q_heads * c.head_dim) % 32 || c.n_layers < 0)
+        return set_err(SAGC_EINVAL, "d_model, d_ff, q_dim must be multiples of 32 and vocab of 16");
+    if (c.page_tokens != 16 && c.page_tokens != 32 && c.page_tokens != 64) return set_err(SAGC_EINVAL, "page_tokens must be 16, 32 or 64");
+    if (c.max_seqs < 1 || c.max_seqs > 1024 || c.n_pages < 1 || c.max_ctx < 2) return set_err(SAGC_EINVAL, "bad max_seqs / n_pages / max_ctx");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return set_err(SAGC_ECUDA, "no CUDA device (there is no CPU fallback)");
+
+    sagc_model* m = new sagc_model();
+    m->cfg = c;
+    const int L = c.n_layers;
+    auto cp = [&](std::vector<const bf16_t*>& v, const void* const* src) {
+        v.resize(L);
+        for (int l = 0; l < L; ++l) v[l] = reinterpret_cast<const bf16_t*>(src[l]);
+    };
+    if (L > 0) { cp(m->wq, w->wq); cp(m->wk, w->wk); cp(m->wv, w->wv); cp(m->wo, w->wo); cp(m->wg, w->wg);
+                 cp(m->wu, w->wu); cp(m->wd, w->wd); cp(m->norm1, w->norm1); cp(m->norm2, w->norm2); }
+    m->embed = reinterpret_cast<const bf16_t*>(w->embed);
+    m->lm_head = reinterpret_cast<const bf16_t*>(w->lm_head);
+    m->final_norm = reinterpret_cast<const bf16_t*>(w->final_norm);
+    m->Nqkv = (c.n_q_heads + 2 * c.n_kv_heads) * c.head_dim;
+    m->max_blocks = (c.max_ctx + c.page_tokens - 1) / c.page_tokens;
+    m->max_rows = c.max_seqs > PREFILL_ROWS ? c.max_seqs : PREFILL_ROWS;
+    m->max_splits = 64;
+    m->page_elems = (size_t)2 * c.n_kv_heads * c.page_tokens * c.head_dim;
+    m->layer_stride = m->page_elems * (size_t)c.n_pages;
+    m->use_pdl = env_int("SAGC_PDL", 1) != 0;
+    m->gemv_max = env_int("SAGC_GEMV_MAX", 0);
+    m->tok_buf = m->len_buf = m->forced_len_d = m->dump_list_d = m->prompt_tok_d = nullptr;
+    m->tok_cap = m->forced_cap = m->dump_cap = m->prompt_cap = 0;
+    m->row_cap = 0;
+    m->row_sid = m->row_pos = m->row_ctx = m->row_tok = nullptr;
+
+    DA(m->kv_pool, m->layer_stride * (size_t)(L > 0 ? L : 1));
+    // RoPE table: angle = pos * theta^(-2i/hd) and cos/sin in fp64 on the host, stored as fp32
+    {
+        const int half = c.head_dim / 2;
+        std::vector<float> cs((size_t)c.max_ctx * half * 2);
+        std::vector<double> inv(half);
+        for (int i = 0; i < half; ++i) inv[i] = pow((double)c.rope_theta, -(2.0 * i) / (double)c.head_dim);
+        for (int p = 0; p < c.max_ctx; ++p)
+            for (int i = 0; i < half; ++i) {
+                const double ang = (double)p * inv[i];
+                cs[((size_t)p * half + i) * 2] = (float)cos(ang);
+                cs[((size_t)p * half + i) * 2 + 1] = (float)sin(ang);
+            }
+        DA(m->rope_cs, cs.size());
+        cudaError_t e = cudaMemcpy(m->rope_cs, cs.data(), cs.size() * sizeof(float), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { sagc_model_destroy(m); return set_err(SAGC_ECUDA, "rope upload: %s", cudaGetErrorString(e)); }
+    }
+    PageState& ps = m->ps;
+    ps.n_pages = c.n_pages; ps.max_blocks = m->max_blocks; ps.page = c.page_tokens; ps.max_seqs = c.max_seqs;
+    ps.log_cap_alloc = c.n_pages * 16 + 65536; ps.log_cap_retire = c.max_seqs;
+    DA(ps.free_stack, c.n_pages); DA(ps.refcnt, c.n_pages);
+    DA(ps.page_table, (size_t)c.max_seqs * m->max_blocks);
+    DA(ps.n_blocks, c.max_seqs); DA(ps.n_shared, c.max_seqs); DA(ps.live, c.max_seqs);
+    DA(ps.pos, c.max_seqs); DA(ps.ctx, c.max_seqs); DA(ps.tok, c.max_seqs);
+    int* scal = nullptr;
+    DA(scal, 16);
+    ps.n_free = scal; ps.n_live = scal + 1; ps.step = scal + 2; ps.err = scal + 3; ps.peak_used = scal + 4;
+    ps.n_alloc = scal + 5; ps.n_retire = scal + 6;
+    DA(ps.alloc_log, (size_t)ps.log_cap_alloc * 3); DA(ps.retire_log, (size_t)ps.log_cap_retire * 2);
+    cudaMemset(scal, 0, 16 * sizeof(int));
+
+    const size_t R = m->max_rows;
+    DA(m->x, R * c.d_model); DA(m->qkv, R * m->Nqkv); DA(m->att, R * c.n_q_heads * c.head_dim);
+    DA(m->act, R * c.d_ff);
+    DA(m->logits, (size_t)c.max_seqs * c.vocab);
+    DA(m->xlast, (size_t)c.max_seqs * c.d_model);
+    DA(m->part_o, (size_t)c.max_seqs * c.n_q_heads * m->max_splits * c.head_dim);
+    DA(m->part_ml, (size_t)c.max_seqs * c.n_q_heads * m->max_splits * 2);
+    DA(m->counters, R * c.n_kv_heads);
+    cudaMemset(m->counters, 0, R * c.n_kv_heads * sizeof(int));
+    DA(m->sampled, c.max_seqs); DA(m->last_idx, c.max_seqs); DA(m->prompt_len_d, c.max_seqs);
+    DA(m->offs_d, c.max_seqs + 1);
+    DA(m->sample_params_d, 4);
+    m->last_nseq = 0; m->last_max_blocks = m->max_blocks;
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) { sagc_model_destroy(m); return set_err(SAGC_ECUDA, "create: %s", cudaGetErrorString(e)); }
+    *out = m;
+    return SAGC_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// forward pass over `m_max` activation rows (decode: live slots; prefill: prompt positions)
+// ---------------------------------------------------------------------------------------
+struct RowSet {
+    const int* sid; const int* pos; const int* ctx; const int* tok; const int* m_dev; int m_max;
+};
+
+static int pick_kind(const sagc_model* m, int path, int m_max) {
+    if (path == SAGC_PATH_GEMV) return LIN_GEMV;
+    if (path == SAGC_PATH_GEMM) return LIN_MMA;
+    return (m_max <= m->gemv_max) ? LIN_GEMV : LIN_MMA;
+}
+
+// layers only (x ends up holding the final residual stream).  Returns kernels launched or <0.
+static int enqueue_layers(sagc_model* m, const RowSet& rs, int n_splits, int kind, cudaStream_t st) {
+    const sagc_model_config& c = m->cfg;
+    int n = 0, r;
+#define LAUNCH(expr) do { r = (expr); if (r < 0) return -1; n += r; } while (0)
+    LAUNCH(launch_embed(m->embed, rs.tok, rs.m_dev, rs.m_max, c.d_model, m->x, st));
+    const int qd = c.n_q_heads * c.head_dim, kvd = c.n_kv_heads * c.head_dim;
+    for (int l = 0; l < c.n_layers; ++l) {
+        LinearArgs a = {};
+        a.W[0] = m->wq[l]; a.W[1] = m->wk[l]; a.W[2] = m->wv[l];
+        a.rows[0] = qd; a.rows[1] = kvd; a.rows[2] = kvd;
+        a.X = m->x; a.norm_w = m->norm1[l]; a.eps = c.rms_eps; a.Y = m->qkv; a.R = nullptr; a.ldy = m->Nqkv;
+        a.K = c.d_model; a.N = m->Nqkv; a.m_dev = rs.m_dev; a.m_max = rs.m_max; a.epi = EPI_STORE; a.kind = kind;
+        a.pdl = m->use_pdl;
+        LAUNCH(launch_linear(a, st));
+
+        RopeArgs ra = {};
+        ra.qkv = m->qkv; ra.row_sid = rs.sid; ra.row_pos = rs.pos; ra.m_dev = rs.m_dev; ra.m_max = rs.m_max;
+        ra.rope_cs = m->rope_cs; ra.kv_layer = m->kv_pool + (size_t)l * m->layer_stride;
+        ra.page_table = m->ps.page_table; ra.max_blocks = m->max_blocks; ra.page = c.page_tokens;
+        ra.Hq = c.n_q_heads; ra.Hkv = c.n_kv_heads; ra.hd = c.head_dim;
+        LAUNCH(launch_rope_append(ra, st));
+
+        AttnArgs aa = {};
+        aa.q = m->qkv; aa.ldq = m->Nqkv; aa.kv_layer = ra.kv_layer; aa.page_table = m->ps.page_table;
+        aa.max_blocks = m->max_blocks; aa.row_sid = rs.sid; aa.row_ctx = rs.ctx; aa.m_dev = rs.m_dev; aa.m_max = rs.m_max;
+        aa.Hq = c.n_q_heads; aa.Hkv = c.n_kv_heads; aa.hd = c.head_dim; aa.page = c.page_tokens;
+        aa.n_splits = n_splits; aa.part_o = m->part_o; aa.part_ml = m->part_ml; aa.counters = m->counters;
+        aa.out = m->att;
+        LAUNCH(launch_attention(aa, st));
+
+        LinearArgs o = {};
+        o.W[0] = m->wo[l]; o.rows[0] = c.d_model; o.X = m->att; o.Y = m->x; o.R = m->x; o.ldy = c.d_model;
+        o.K = qd; o.N = c.d_model; o.m_dev = rs.m_dev; o.m_max = rs.m_max; o.epi = EPI_RESID; o.kind = kind;
+        o.pdl = m->use_pdl; o.eps = c.rms_eps;
+        LAUNCH(launch_linear(o, st));
+
+        LinearArgs gu = {};
+        gu.W[0] = m->wg[l]; gu.W[1] = m->wu[l]; gu.rows[0] = c.d_ff; gu.rows[1] = c.d_ff;
+        gu.X = m->x; gu.norm_w = m->norm2[l]; gu.eps = c.rms_eps; gu.Y = m->act; gu.ldy = c.d_ff;
+        gu.K = c.d_model; gu.N = c.d_ff; gu.m_dev = rs.m_dev; gu.m_max = rs.m_max; gu.epi = EPI_SWIGLU; gu.kind = kind;
+        gu.pdl = m->use_pdl;
+        LAUNCH(launch_linear(gu, st));
+
+        LinearArgs dn = {};
+        dn.W[0] = m->wd[l]; dn.rows[0] = c.d_model; dn.X = m->act; dn.Y = m->x; dn.R = m->x; dn.ldy = c.d_model;
+        dn.K = c.d_ff; dn.N = c.d_model; dn.m_dev = rs.m_dev; dn.m_max = rs.m_max; dn.epi = EPI_RESID; dn.kind = kind;
+        dn.pdl = m->use_pdl; dn.eps = c.rms_eps;
+        LAUNCH(launch_linear(dn, st));
+    }
+    return n;
+}
+
+// final norm + LM head over rows of `xsrc` -> m->logits
+static int enqueue_lm_head(sagc_model* m, const float* xsrc, const int* m_dev, int m_max, int kind, cudaStream_t st) {
+    const sagc_model_config& c = m->cfg;
+    LinearArgs a = {};
+    a.W[0] = m->lm_head; a.rows[0] = c.vocab; a.X = xsrc; a.norm_w = m->final_norm; a.eps = c.rms_eps;
+    a.Y = m->logits; a.ldy = c.vocab; a.K = c.d_model; a.N = c.vocab; a.m_dev = m_dev; a.m_max = m_max;
+    a.epi = EPI_STORE; a.kind = kind; a.pdl = m->use_pdl;
+    return launch_linear(a, st);
+}
+
+template <typename T>
+static int grow(sagc_model* m, T** p, size_t* cap, size_t need, bool* changed) {
+    if (need <= *cap && *p) return SAGC_OK;
+    T* q = nullptr;
+    size_t n = need + need / 4 + 64;
+    int rc = dev_alloc(m, &q, n);
+    if (rc != SAGC_OK) return rc;
+    *p = q; *cap = n;      // the old block stays owned by the handle until destroy
+    if (changed) *changed = true;
+    return SAGC_OK;
+}
+
+static int round_bucket(int live) {
+    if (live <= 8) return 8;
+    if (live <= 16) return 16;
+    if (live <= 32) return 32;
+    return ((live + 63) / 64) * 64;
+}
+
+static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
+    const int ctas = m_bucket * m->cfg.n_kv_heads;
+    int want = (2 * 148 + ctas - 1) / ctas;
+    int cap = ctx_bound / 256;
+    if (cap < 1) cap = 1;
+    if (want > cap) want = cap;
+    if (want > m->max_splits) want = m->max_splits;
+    int s = 1;
+    while (s * 2 <= want) s *= 2;
+    return s;
+}
+
+// ---------------------------------------------------------------------------------------
+// sagc_rollout_group
+// ---------------------------------------------------------------------------------------
+static int enqueue_decode_step(sagc_model* m, const RolloutDev& rd, int m_bucket, int n_splits, int kind,
+                               int n_dump, float* dump_out, cudaStream_t st) {
+    RowSet rs = {m->ps.live, m->ps.pos, m->ps.ctx, m->ps.tok, m->ps.n_live, m_bucket};
+    int n = enqueue_layers(m, rs, n_splits, kind, st);
+    if (n < 0) return -1;
+    int r = enqueue_lm_head(m, m->x, m->ps.n_live, m_bucket, kind, st);
+    if (r < 0) return -1;
+    n += r;
+    SampleArgs sa = {};
+    sa.logits = m->logits; sa.V = m->cfg.vocab; sa.row_sid = m->ps.live; sa.step_dev = m->ps.step;
+    sa.m_dev = m->ps.n_live; sa.m_max = m_bucket; sa.params = m->sample_params_d; sa.row_div = 1;
+    sa.out_tok = m->sampled;
+    n += launch_sample(sa, st);
+    if (n_dump > 0)
+        n += launch_dump_logits(m->dump_list_d, n_dump, m->ps.step, m->ps.live, m->ps.n_live, 1, m->logits,
+                                m->cfg.vocab, dump_out, st);
+    n += launch_advance(m->ps, rd, m->sampled, 0, st);
+    return n;
+}
+
+static int phase_of(int live, int nseq) {
+    if (live <= 8 && 2 * live < nseq) return 2;    // TAIL
+    if (2 * live >= nseq) return 0;                // FULL
+    return 1;                                      // MID
+}
+
+extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, const int32_t* prompt_offsets,
+                                  int32_t n_prompts, int32_t G, const sagc_rollout_params* prm,
+                                  int32_t* out_tokens, int32_t* out_lengths, float* out_ratio,
+                                  int32_t* out_len_stats, sagc_rollout_timing* timing, void* stream) {
+    if (!m || !prompt_offsets || !prm || !out_tokens || !out_lengths) return set_err(SAGC_EINVAL, "null argument");
+    const sagc_model_config& c = m->cfg;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const int nseq = n_prompts * G;
+    const int max_new = prm->max_new_tokens;
+    const bool structure_only = (prm->flags & SAGC_FLAG_STRUCTURE_ONLY) != 0;
+    const bool use_graph = !(prm->flags & SAGC_FLAG_NO_GRAPH);
+    if (n_prompts < 1 || G < 1 || nseq > c.max_seqs) return set_err(SAGC_EINVAL, "n_prompts*G = %d exceeds max_seqs = %d", nseq, c.max_seqs);
+    if (max_new < 1) return set_err(SAGC_EINVAL, "max_new_tokens must be >= 1");
+    if (structure_only && !prm->forced_lengths) return set_err(SAGC_EINVAL, "STRUCTURE_ONLY needs forced_lengths");
+    if (!structure_only && !prompt_tokens) return set_err(SAGC_EINVAL, "prompt_tokens is null");
+    if (prm->mode != SAGC_MODE_GREEDY && prm->mode != SAGC_MODE_GUMBEL) return set_err(SAGC_EINVAL, "bad sampling mode");
+    if (prm->mode == SAGC_MODE_GUMBEL && !(prm->temperature > 0.f)) return set_err(SAGC_EINVAL, "temperature must be > 0");
+    if (prompt_offsets[0] != 0) return set_err(SAGC_EINVAL, "prompt_offsets[0] must be 0");
+    std::vector<int> plen(n_prompts);
+    int total_rows = 0, pmax = 0;
+    for (int p = 0; p < n_prompts; ++p) {
+        plen[p] = prompt_offsets[p + 1] - prompt_offsets[p];
+        if (plen[p] < 1) return set_err(SAGC_EINVAL, "prompt %d is empty", p);
+        if (plen[p] + max_new > c.max_ctx) return set_err(SAGC_EINVAL, "prompt %d: length + max_new_tokens exceeds max_ctx", p);
+        total_rows += plen[p];
+        if (plen[p] > pmax) pmax = plen[p];
+    }
+    if (prm->n_dump > 0 && (!prm->dump_sid_t || !prm->dump_logits)) return set_err(SAGC_EINVAL, "dump arrays are null");
+
+    // ---- per-call device buffers ------------------------------------------------------
+    bool changed = false;
+    int rc;
+    if ((rc = grow(m, &m->tok_buf, &m->tok_cap, (size_t)nseq * max_new, &changed)) != SAGC_OK) return rc;
+    if (!m->len_buf) { size_t cap = 0; if ((rc = grow(m, &m->len_buf, &cap, (size_t)c.max_seqs, &changed)) != SAGC_OK) return rc; }
+    if (prm->forced_lengths && (rc = grow(m, &m->forced_len_d, &m->forced_cap, (size_t)nseq, &changed)) != SAGC_OK) return rc;
+    if (prm->n_dump > 0 && (rc = grow(m, &m->dump_list_d, &m->dump_cap, (size_t)prm->n_dump * 2, &changed)) != SAGC_OK) return rc;
+    if (!structure_only) {
+        size_t cap = (size_t)m->row_cap;
+        if ((size_t)total_rows > cap) {
+            size_t c1 = 0, c2 = 0, c3 = 0, c4 = 0;
+            m->row_sid = m->row_pos = m->row_ctx = m->row_tok = nullptr;
+            if ((rc = grow(m, &m->row_sid, &c1, (size_t)total_rows, &changed)) != SAGC_OK) return rc;
+            if ((rc = grow(m, &m->row_pos, &c2, (size_t)total_rows, &changed)) != SAGC_OK) return rc;
+            if ((rc = grow(m, &m->row_ctx, &c3, (size_t)total_rows, &changed)) != SAGC_OK) return rc;
+            if ((rc = grow(m, &m->row_tok, &c4, (size_t)total_rows, &changed)) != SAGC_OK) return rc;
+            m->row_cap = (int)c1;
+        }
+    }
+    CU(cudaMemcpyAsync(m->prompt_len_d, plen.data(), n_prompts * sizeof(int), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(m->offs_d, prompt_offsets, (n_prompts + 1) * sizeof(int), cudaMemcpyHostToDevice, st));
+    if (prm->forced_lengths)
+        CU(cudaMemcpyAsync(m->forced_len_d, prm->forced_lengths, nseq * sizeof(int), cudaMemcpyHostToDevice, st));
+    if (prm->n_dump > 0)
+        CU(cudaMemcpyAsync(m->dump_list_d, prm->dump_sid_t, (size_t)prm->n_dump * 2 * sizeof(int), cudaMemcpyHostToDevice, st));
+    uint32_t sp[4];
+    sp[0] = (uint32_t)prm->mode;
+    float temp = prm->mode == SAGC_MODE_GUMBEL ? prm->temperature : 1.f;
+    memcpy(&sp[1], &temp, 4);
+    sp[2] = (uint32_t)(prm->seed & 0xffffffffull); sp[3] = (uint32_t)(prm->seed >> 32);
+    CU(cudaMemcpyAsync(m->sample_params_d, sp, sizeof(sp), cudaMemcpyHostToDevice, st));
+
+    RolloutDev rd = {};
+    rd.prompt_len = m->prompt_len_d;
+    rd.forced_len = prm->forced_lengths ? m->forced_len_d : nullptr;
+    rd.forced_tok = prm->forced_tokens;
+    rd.out_tokens = m->tok_buf; rd.out_lengths = m->len_buf;
+    rd.n_prompts = n_prompts; rd.G = G; rd.nseq = nseq; rd.max_new = max_new; rd.stop_token = prm->stop_token;
+    rd.log = (prm->flags & SAGC_FLAG_LOG) ? 1 : 0;
+
+    // graphs bake every kernel argument: they are valid for one signature only
+    char sig[256];
+    snprintf(sig, sizeof(sig), "%d/%d/%d/%d/%d/%p/%p/%p/%d/%p/%d", n_prompts, G, max_new, prm->stop_token, rd.log,
+             (const void*)rd.forced_len, (const void*)rd.forced_tok, (const void*)m->tok_buf, prm->n_dump,
+             (const void*)prm->dump_logits, (int)m->use_pdl);
+    if (changed || m->signature != sig) { clear_graphs(m); m->signature = sig; }
+    m->last_nseq = nseq;
+
+    // ---- host-side schedule -------------------------------------------------------------
+    // With forced lengths the live count of every step is known in advance.
+    std::vector<int> eff(nseq, max_new);
+    if (prm->forced_lengths)
+        for (int i = 0; i < nseq; ++i) { int f = prm->forced_lengths[i]; eff[i] = (f >= 1 && f < max_new) ? f : max_new; }
+    int t_last = 0;
+    for (int i = 0; i < nseq; ++i) if (eff[i] > t_last) t_last = eff[i];
+    std::vector<int> live_at(t_last + 2, 0), glive_at;     // live_at[t] = #{eff >= t}
+    {
+        std::vector<int> cnt(t_last + 2, 0);
+        for (int i = 0; i < nseq; ++i) cnt[eff[i]]++;
+        int run = 0;
+        for (int t = t_last; t >= 1; --t) { run += cnt[t]; live_at[t] = run; }
+        glive_at.assign(t_last + 2, 0);
+        std::vector<int> gcnt(t_last + 2, 0);
+        for (int p = 0; p < n_prompts; ++p) { int mx = 0; for (int g = 0; g < G; ++g) mx = eff[p * G + g] > mx ? eff[p * G + g] : mx; gcnt[mx]++; }
+        run = 0;
+        for (int t = t_last; t >= 1; --t) { run += gcnt[t]; glive_at[t] = run; }
+    }
+    const bool known = prm->forced_lengths != nullptr && prm->stop_token < 0;
+
+    const bool want_t = timing != nullptr;
+    if (want_t) memset(timing, 0, sizeof(*timing));
+    cudaEvent_t ev[8];
+    int n_ev = 0;
+    auto mark = [&]() -> cudaEvent_t { cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, st); ev[n_ev++] = e; return e; };
+    long long launches = 0;
+    int r;
+
+    // ---- a1: pool reset + prefix pages ----------------------------------------------------
+    launches += launch_pool_reset(m->ps, rd, st);
+    launches += launch_prefill_alloc(m->ps, rd, st);
+    cudaEvent_t e_start = nullptr, e_pf = nullptr;
+    if (want_t) e_start = mark();
+
+    if (!structure_only) {
+        // ---- a2: prefill, once per prompt, in row chunks ----------------------------------
+        const int* ptok = prompt_tokens;      // device pointer supplied by the caller
+        launches += launch_prefill_rows(ptok, m->offs_d, n_prompts, G, total_rows, m->row_sid, m->row_pos, m->row_ctx,
+                                        m->row_tok, st);
+        const int kind_pf = pick_kind(m, prm->path, PREFILL_ROWS);
+        std::vector<int> idx;
+        for (int r0 = 0; r0 < total_rows; r0 += PREFILL_ROWS) {
+            const int rows = (total_rows - r0) < PREFILL_ROWS ? (total_rows - r0) : PREFILL_ROWS;
+            RowSet rs = {m->row_sid + r0, m->row_pos + r0, m->row_ctx + r0, m->row_tok + r0, nullptr, rows};
+            r = enqueue_layers(m, rs, 1, kind_pf, st);
+            if (r < 0) return set_err(SAGC_ECUDA, "prefill launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+            launches += r;
+            // last row of every prompt that ends inside this chunk -> xlast[p]
+            idx.clear();
+            int p_first = -1;
+            for (int p = 0; p < n_prompts; ++p) {
+                const int last = prompt_offsets[p + 1] - 1 - prompt_offsets[0];
+                if (last >= r0 && last < r0 + rows) { if (p_first < 0) p_first = p; idx.push_back(last - r0); }
+            }
+            if (!idx.empty()) {
+                CU(cudaMemcpyAsync(m->last_idx + p_first, idx.data(), idx.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+                CU(cudaStreamSynchronize(st));       // idx is reused by the next chunk
+                launches += launch_gather_rows(m->x, m->last_idx + p_first, (int)idx.size(), c.d_model,
+                                               m->xlast + (size_t)p_first * c.d_model, st);
+            }
+        }
+        launches += launch_copy_partial_block(m->ps, rd, m->kv_pool, m->layer_stride, c.n_layers > 0 ? c.n_layers : 0,
+                                              (int)m->page_elems, st);
+        // ---- a3: first token of each completion from its prompt's last-row logits -----------
+        r = enqueue_lm_head(m, m->xlast, nullptr, n_prompts, pick_kind(m, prm->path, n_prompts), st);
+        if (r < 0) return set_err(SAGC_ECUDA, "lm head launch failed");
+        launches += r;
+        SampleArgs sa = {};
+        sa.logits = m->logits; sa.V = c.vocab; sa.row_sid = m->ps.live; sa.step_dev = m->ps.step;
+        sa.m_dev = m->ps.n_live; sa.m_max = nseq; sa.params = m->sample_params_d; sa.row_div = G; sa.out_tok = m->sampled;
+        launches += launch_sample(sa, st);
+        if (prm->n_dump > 0)
+            launches += launch_dump_logits(m->dump_list_d, prm->n_dump, m->ps.step, m->ps.live, m->ps.n_live, G,
+                                           m->logits, c.vocab, prm->dump_logits, st);
+    }
+    launches += launch_advance(m->ps, rd, m->sampled, structure_only ? 1 : 0, st);     // end of step 1
+    if (want_t) e_pf = mark();
+
+    // ---- decode loop: steps t = 2 .. ---------------------------------------------------
+    const double Wb = 2.0 * ((double)c.n_layers * ((double)c.d_model * c.n_q_heads * c.head_dim * 2 +
+                                                   2.0 * c.d_model * c.n_kv_heads * c.head_dim + 3.0 * c.d_model * c.d_ff) +
+                             (double)c.vocab * c.d_model);
+    const double KVB = 2.0 * c.n_layers * c.n_kv_heads * c.head_dim * 2.0;
+    int cur_phase = -1;
+    cudaEvent_t ph_start[3] = {nullptr, nullptr, nullptr}, ph_end[3] = {nullptr, nullptr, nullptr};
+    int live_bound = nseq;
+    int t = 2;
+    while (true) {
+        int live;
+        if (known) {
+            if (t > t_last) break;
+            live = live_at[t];
+        } else {
+            if (t > max_new) break;
+            if ((t - 2) % 16 == 0) {          // poll the device's live count
+                int h[2];
+                CU(cudaMemcpyAsync(h, m->ps.n_live, sizeof(int), cudaMemcpyDeviceToHost, st));
+                CU(cudaMemcpyAsync(h + 1, m->ps.err, sizeof(int), cudaMemcpyDeviceToHost, st));
+                CU(cudaStreamSynchronize(st));
+                live_bound = h[0];
+                if (h[1] || live_bound == 0) break;
+            }
+            live = live_bound;
+        }
+        if (live == 0) break;
+        const int ph = phase_of(live, nseq);
+        if (want_t && ph != cur_phase) {
+            cudaEvent_t e = mark();
+            if (cur_phase >= 0) ph_end[cur_phase] = e;
+            if (!ph_start[ph]) ph_start[ph] = e;
+            cur_phase = ph;
+        }
+        if (want_t) {
+            timing->phase_steps[ph] += 1;
+            timing->phase_tokens[ph] += live;
+            const double gl = known ? glive_at[t] : n_prompts;
+            timing->phase_bytes[ph] += Wb + KVB * (gl * (double)pmax + (double)live * (t - 1)) + KVB * live;
+        }
+        if (structure_only) {
+            launches += launch_advance(m->ps, rd, m->sampled, 1, st);
+        } else {
+            const int mb = round_bucket(live);
+            const int ns = pick_splits(m, mb, pmax + t - 1);
+            const int kind = pick_kind(m, prm->path, mb);
+            if (use_graph) {
+                GraphKey key = {mb, ns, kind, prm->n_dump};
+                auto it = m->graphs.find(key);
+                if (it == m->graphs.end()) {
+                    cudaGraph_t g;
+                    CU(cudaStreamBeginCapture(st, cudaStreamCaptureModeRelaxed));
+                    int nk = enqueue_decode_step(m, rd, mb, ns, kind, prm->n_dump, prm->dump_logits, st);
+                    cudaError_t ce = cudaStreamEndCapture(st, &g);
+                    if (nk < 0 || ce != cudaSuccess) return set_err(SAGC_ECUDA, "graph capture failed: %s", cudaGetErrorString(ce));
+                    GraphVal gv;
+                    gv.n_kernels = nk;
+                    CU(cudaGraphInstantiate(&gv.exec, g, 0));
+                    cudaGraphDestroy(g);
+                    it = m->graphs.emplace(key, gv).first;
+                }
+                CU(cudaGraphLaunch(it->second.exec, st));
+                launches += it->second.n_kernels;
+            } else {
+                r = enqueue_decode_step(m, rd, mb, ns, kind, prm->n_dump, prm->dump_logits, st);
+                if (r < 0) return set_err(SAGC_ECUDA, "decode launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+                launches += r;
+            }
+        }
+        ++t;
+    }
+    cudaEvent_t e_end = nullptr;
+    if (want_t) { e_end = mark(); if (cur_phase >= 0) ph_end[cur_phase] = e_end; }
+
+    // ---- a14: length statistics, outputs ---------------------------------------------------
+    // group offsets = p*G: reuse offs_d (prompt offsets are no longer needed on the device)
+    {
+        std::vector<int> goffs(n_prompts + 1);
+        for (int p = 0; p <= n_prompts; ++p) goffs[p] = p * G;
+        CU(cudaMemcpyAsync(m->offs_d, goffs.data(), (n_prompts + 1) * sizeof(int), cudaMemcpyHostToDevice, st));
+        CU(cudaStreamSynchronize(st));
+    }
+    if (out_ratio || out_len_stats)
+        launches += launch_length_stats(m->len_buf, m->offs_d, n_prompts, out_len_stats, out_ratio, st);
+    CU(cudaMemcpyAsync(out_tokens, m->tok_buf, (size_t)nseq * max_new * sizeof(int), cudaMemcpyDeviceToDevice, st));
+    CU(cudaMemcpyAsync(out_lengths, m->len_buf, (size_t)nseq * sizeof(int), cudaMemcpyDeviceToDevice, st));
+    int herr = 0;
+    CU(cudaMemcpyAsync(&herr, m->ps.err, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    if (want_t) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e_start, e_pf); timing->prefill_ms = ms;
+        cudaEventElapsedTime(&ms, e_pf, e_end); timing->decode_ms = ms;
+        for (int p = 0; p < 3; ++p)
+            if (ph_start[p] && ph_end[p]) { cudaEventElapsedTime(&ms, ph_start[p], ph_end[p]); timing->phase_ms[p] = ms; }
+        timing->prefill_tokens = structure_only ? 0 : total_rows;
+        timing->prefill_flops = structure_only ? 0.0 : (double)total_rows * Wb;   // 2 flop per bf16 weight per row (+attention, not counted)
+        long long tot = 0;
+        for (int i = 0; i < nseq; ++i) tot += known ? eff[i] : 0;
+        timing->total_tokens = tot;
+        timing->kernel_launches = launches;
+    }
+    for (int i = 0; i < n_ev; ++i) cudaEventDestroy(ev[i]);
+    if (herr) return set_err(SAGC_EPAGES, "KV page pool exhausted (n_pages = %d)", c.n_pages);
+    return SAGC_OK;
+}
+
+extern "C" int sagc_rollout_group_host(sagc_model* m, const int32_t* prompt_tokens, const int32_t* prompt_offsets,
+                                       int32_t n_prompts, int32_t G, const sagc_rollout_params* prm,
+                                       int32_t* out_tokens, int32_t* out_lengths, float* out_ratio,
+                                       int32_t* out_len_stats, sagc_rollout_timing* timing, void* stream) {
+    if (!m || !prompt_offsets || !prm || !out_tokens || !out_lengths) return set_err(SAGC_EINVAL, "null argument");
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const int nseq = n_prompts * G;
+    if (n_prompts < 1 || G < 1 || prm->max_new_tokens < 1) return set_err(SAGC_EINVAL, "bad sizes");
+    const size_t ntok = (size_t)nseq * prm->max_new_tokens;
+    const int total = prompt_offsets[n_prompts];
+    int *d_prompt = nullptr, *d_tok = nullptr, *d_len = nullptr, *d_stats = nullptr;
+    float* d_ratio = nullptr;
+    int rc = SAGC_OK;
+    auto fail = [&](int code) {
+        cudaFree(d_prompt); cudaFree(d_tok); cudaFree(d_len); cudaFree(d_stats); cudaFree(d_ratio);
+        return code;
+    };
+#define CUH(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return fail(set_err(SAGC_ECUDA, "%s: %s", #x, cudaGetErrorString(e_))); } while (0)
+    CUH(cudaMalloc(&d_prompt, (size_t)(total > 0 ? total : 1) * sizeof(int)));
+    CUH(cudaMalloc(&d_tok, ntok * sizeof(int)));
+    CUH(cudaMalloc(&d_len, (size_t)nseq * sizeof(int)));
+    CUH(cudaMalloc(&d_stats, (size_t)n_prompts * 3 * sizeof(int)));
+    CUH(cudaMalloc(&d_ratio, (size_t)n_prompts * sizeof(float)));
+    if (prompt_tokens && total > 0)
+        CUH(cudaMemcpyAsync(d_prompt, prompt_tokens, (size_t)total * sizeof(int), cudaMemcpyHostToDevice, st));
+    rc = sagc_rollout_group(m, prompt_tokens ? d_prompt : nullptr, prompt_offsets, n_prompts, G, prm, d_tok, d_len,
+                            d_ratio, d_stats, timing, stream);
+    if (rc != SAGC_OK) return fail(rc);
+    CUH(cudaMemcpyAsync(out_tokens, d_tok, ntok * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUH(cudaMemcpyAsync(out_lengths, d_len, (size_t)nseq * sizeof(int), cudaMemcpyDeviceToHost, st));
+    if (out_ratio) CUH(cudaMemcpyAsync(out_ratio, d_ratio, (size_t)n_prompts * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (out_len_stats) CUH(cudaMemcpyAsync(out_len_stats, d_stats, (size_t)n_prompts * 3 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUH(cudaStreamSynchronize(st));
+    fail(0);
+    return SAGC_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// group statistics
+// ---------------------------------------------------------------------------------------
+extern "C" int sagc_group_advantage(const float* rewards, const int32_t* group_offsets, int32_t n_groups, int32_t mode,
+                                    int32_t ddof, float eps, float* out_adv, uint8_t* out_keep, void* stream) {
+    if (n_groups < 0 || (n_groups > 0 && (!rewards || !group_offsets || !out_adv || !out_keep)))
+        return set_err(SAGC_EINVAL, "null argument");
+    if (mode != SAGC_ADV_GRPO && mode != SAGC_ADV_DAPO) return set_err(SAGC_EINVAL, "mode must be GRPO or DAPO");
+    if (ddof != 0 && ddof != 1) return set_err(SAGC_EINVAL, "ddof must be 0 or 1");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return set_err(SAGC_ECUDA, "no CUDA device (there is no CPU fallback)");
+    launch_group_advantage(rewards, group_offsets, n_groups, mode, ddof, eps, out_adv, out_keep,
+                           reinterpret_cast<cudaStream_t>(stream));
+    CU(cudaGetLastError());
+    return SAGC_OK;
+}
+
+extern "C" int sagc_length_stats(const int32_t* lengths, const int32_t* group_offsets, int32_t n_groups,
+                                 int32_t* out_stats, float* out_ratio, void* stream) {
+    if (n_groups < 0 || (n_groups > 0 && (!lengths || !group_offsets))) return set_err(SAGC_EINVAL, "null argument");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return set_err(SAGC_ECUDA, "no CUDA device (there is no CPU fallback)");
+    launch_length_stats(lengths, group_offsets, n_groups, out_stats, out_ratio, reinterpret_cast<cudaStream_t>(stream));
+    CU(cudaGetLastError());
+    return SAGC_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// debug / parity exports
+// ---------------------------------------------------------------------------------------
+extern "C" int sagc_debug_page_table(sagc_model* m, int32_t* out, int32_t capacity, int32_t* nseq, int32_t* max_blocks) {
+    if (!m || !out) return set_err(SAGC_EINVAL, "null argument");
+    const int n = m->last_nseq, mb = m->max_blocks;
+    if (nseq) *nseq = n;
+    if (max_blocks) *max_blocks = mb;
+    if ((long long)n * mb > capacity) return set_err(SAGC_EINVAL, "capacity %d < %lld", capacity, (long long)n * mb);
+    CU(cudaDeviceSynchronize());
+    CU(cudaMemcpy(out, m->ps.page_table, (size_t)n * mb * sizeof(int), cudaMemcpyDeviceToHost));
+    return SAGC_OK;
+}
+extern "C" int sagc_debug_free_stack(sagc_model* m, int32_t* out, int32_t capacity, int32_t* n_free) {
+    if (!m || !out || !n_free) return set_err(SAGC_EINVAL, "null argument");
+    CU(cudaDeviceSynchronize());
+    CU(cudaMemcpy(n_free, m->ps.n_free, sizeof(int), cudaMemcpyDeviceToHost));
+    if (*n_free > capacity) return set_err(SAGC_EINVAL, "capacity too small");
+    CU(cudaMemcpy(out, m->ps.free_stack, (size_t)(*n_free) * sizeof(int), cudaMemcpyDeviceToHost));
+    return SAGC_OK;
+}
+static int copy_log(const int* dev_log, const int* dev_n, int width, int cap_entries, int32_t* out, int32_t capacity, int32_t* n) {
+    if (!out || !n) return set_err(SAGC_EINVAL, "null argument");
+    CU(cudaDeviceSynchronize());
+    CU(cudaMemcpy(n, dev_n, sizeof(int), cudaMemcpyDeviceToHost));
+    int k = *n < cap_entries ? *n : cap_entries;
+    if (k > capacity) return set_err(SAGC_EINVAL, "capacity %d < %d entries", capacity, k);
+    CU(cudaMemcpy(out, dev_log, (size_t)k * width * sizeof(int), cudaMemcpyDeviceToHost));
+    return SAGC_OK;
+}
+extern "C" int sagc_debug_alloc_log(sagc_model* m, int32_t* out, int32_t capacity, int32_t* n) {
+    if (!m) return set_err(SAGC_EINVAL, "null argument");
+    return copy_log(m->ps.alloc_log, m->ps.n_alloc, 3, m->ps.log_cap_alloc, out, capacity, n);
+}
+extern "C" int sagc_debug_retire_log(sagc_model* m, int32_t* out, int32_t capacity, int32_t* n) {
+    if (!m) return set_err(SAGC_EINVAL, "null argument");
+    return copy_log(m->ps.retire_log, m->ps.n_retire, 2, m->ps.log_cap_retire, out, capacity, n);
+}
+extern "C" int sagc_debug_peak_pages(sagc_model* m, int32_t* peak) {
+    if (!m || !peak) return set_err(SAGC_EINVAL, "null argument");
+    CU(cudaDeviceSynchronize());
+    CU(cudaMemcpy(peak, m->ps.peak_used, sizeof(int), cudaMemcpyDeviceToHost));
+    return SAGC_OK;
+}
+extern "C" int sagc_debug_philox(uint64_t seed, int32_t sid, int32_t t, int32_t v0, int32_t n, uint32_t* out, void* stream) {
+    if (n < 0 || (n > 0 && !out)) return set_err(SAGC_EINVAL, "null argument");
+    launch_philox_debug(seed, sid, t, v0, n, out, reinterpret_cast<cudaStream_t>(stream));
+    CU(cudaGetLastError());
+    return SAGC_OK;
+}
+extern "C" int sagc_debug_linear(const void* W, const float* x, float* y, int32_t M, int32_t N, int32_t K, int32_t path,
+                                 void* stream) {
+    if (!W || !x || !y || M < 1 || N % 16 || K % 32) return set_err(SAGC_EINVAL, "need N %% 16 == 0 and K %% 32 == 0");
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    // rows beyond 64 are processed by the kernels' own m-chunk grid dimension
+    LinearArgs a = {};
+    a.W[0] = reinterpret_cast<const bf16_t*>(W); a.rows[0] = N; a.X = x; a.Y = y; a.ldy = N; a.K = K; a.N = N;
+    a.m_dev = nullptr; a.m_max = M; a.epi = EPI_STORE; a.kind = (path == SAGC_PATH_GEMV) ? LIN_GEMV : LIN_MMA; a.pdl = false;
+    if (launch_linear(a, st) < 0) return set_err(SAGC_ECUDA, "launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    CU(cudaGetLastError());
+    return SAGC_OK;
+}
+extern "C" int sagc_debug_attention(const float* q, const void* kv, const int32_t* page_table, const int32_t* ctx, int32_t M,
+                                    int32_t Hq, int32_t Hkv, int32_t hd, int32_t page_tokens, int32_t max_blocks, float* out,
+                                    void* stream) {
+    if (!q || !kv || !page_table || !ctx || !out || M < 1) return set_err(SAGC_EINVAL, "null argument");
+    if (Hq % Hkv || Hq / Hkv > 8) return set_err(SAGC_EINVAL, "bad head counts");
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const int n_splits = env_int("SAGC_DEBUG_SPLITS", 4);
+    int *sid = nullptr, *cnt = nullptr;
+    float *po = nullptr, *pml = nullptr;
+    CU(cudaMalloc(&sid, M * sizeof(int)));
+    CU(cudaMalloc(&cnt, (size_t)M * Hkv * sizeof(int)));
+    CU(cudaMalloc(&po, (size_t)M * Hq * n_splits * hd * sizeof(float)));
+    CU(cudaMalloc(&pml, (size_t)M * Hq * n_splits * 2 * sizeof(float)));
+    std::vector<int> ident(M);
+    for (int i = 0; i < M; ++i) ident[i] = i;
+    CU(cudaMemcpyAsync(sid, ident.data(), M * sizeof(int), cudaMemcpyHostToDevice, st));
+    CU(cudaMemsetAsync(cnt, 0, (size_t)M * Hkv * sizeof(int), st));
+    AttnArgs a = {};
+    a.q = q; a.ldq = Hq * hd; a.kv_layer = reinterpret_cast<const bf16_t*>(kv); a.page_table = page_table;
+    a.max_blocks = max_blocks; a.row_sid = sid; a.row_ctx = ctx; a.m_dev = nullptr; a.m_max = M; a.Hq = Hq; a.Hkv = Hkv;
+    a.hd = hd; a.page = page_tokens; a.n_splits = n_splits; a.part_o = po; a.part_ml = pml; a.counters = cnt; a.out = out;
+    int r = launch_attention(a, st);
+    cudaError_t e = cudaStreamSynchronize(st);
+    cudaFree(sid); cudaFree(cnt); cudaFree(po); cudaFree(pml);
+    if (r < 0) return set_err(SAGC_EINVAL, "unsupported head_dim %d", hd);
+    if (e != cudaSuccess) return set_err(SAGC_ECUDA, "attention: %s", cudaGetErrorString(e));
+    return SAGC_OK;
+}

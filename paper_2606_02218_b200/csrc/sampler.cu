@@ -1,0 +1,140 @@
+// sampler.cu -- greedy / Philox-keyed Gumbel-max sampler (steps a3, a12).
+//   Philox4x32-10, key = (seed lo, seed hi), counter = (v >> 2, t, sid, 0); word v & 3 is the
+//   draw for vocab id v.  u = ((x >> 9) + 0.5) * 2^-23;  g = -log(-log u);
+//   token = argmax_v(logit_v / T + g_v), lowest v on exact ties (reading C2).
+#include "common.cuh"
+#include "kernels.cuh"
+
+namespace sagc {
+
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                              uint32_t k1, uint32_t (&out)[4]) {
+#pragma unroll
+    for (int i = 0; i < 10; ++i) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+__device__ __forceinline__ float gumbel_from_u32(uint32_t x) {
+    const float u = ((float)(x >> 9) + 0.5f) * 1.1920928955078125e-07f;   // 2^-23, exact in fp32
+    return -logf(-logf(u));
+}
+
+__global__ void k_philox_debug(uint32_t k0, uint32_t k1, int sid, int t, int v0, int n, uint32_t* out) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int v = v0 + i;
+    uint32_t w[4];
+    philox4x32_10((uint32_t)v >> 2, (uint32_t)t, (uint32_t)sid, 0u, k0, k1, w);
+    out[i] = w[v & 3];
+}
+int launch_philox_debug(uint64_t seed, int sid, int t, int v0, int n, uint32_t* out, cudaStream_t st) {
+    if (n <= 0) return 0;
+    k_philox_debug<<<(n + 255) / 256, 256, 0, st>>>((uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32), sid, t,
+                                                    v0, n, out);
+    return 1;
+}
+
+static constexpr int SMP_THREADS = 1024;
+
+__device__ __forceinline__ void better(float& bs, int& bi, float s, int i) {
+    if (s > bs || (s == bs && i < bi)) { bs = s; bi = i; }
+}
+
+// one CTA per row
+__global__ void __launch_bounds__(SMP_THREADS) k_sample(SampleArgs a) {
+    __shared__ float ws[32];
+    __shared__ int wi[32];
+    pdl_wait();
+    pdl_launch();
+    const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
+    const int row = blockIdx.x;
+    if (row >= M) return;
+    const float* lg = a.logits + (size_t)(row / a.row_div) * a.V;
+    const int sid = a.row_sid[row];
+    const int mode = (int)a.params[0];
+    const float temperature = __uint_as_float(a.params[1]);
+    const uint32_t k0 = a.params[2], k1 = a.params[3];
+    const int t = *a.step_dev;
+    float bs = -INFINITY;
+    int bi = 0x7fffffff;
+    const int nblk = (a.V + 3) >> 2;
+    for (int b = threadIdx.x; b < nblk; b += SMP_THREADS) {
+        const int v = b << 2;
+        float s[4];
+        if (v + 3 < a.V) {
+            float4 x = __ldcs(reinterpret_cast<const float4*>(lg + v));
+            s[0] = x.x; s[1] = x.y; s[2] = x.z; s[3] = x.w;
+        } else {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) s[e] = (v + e < a.V) ? lg[v + e] : -INFINITY;
+        }
+        if (mode == 1) {
+            uint32_t w[4];
+            philox4x32_10((uint32_t)b, (uint32_t)t, (uint32_t)sid, 0u, k0, k1, w);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) s[e] = s[e] / temperature + gumbel_from_u32(w[e]);
+        }
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+            if (v + e < a.V) better(bs, bi, s[e], v + e);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        float s2 = __shfl_xor_sync(0xffffffffu, bs, o);
+        int i2 = __shfl_xor_sync(0xffffffffu, bi, o);
+        better(bs, bi, s2, i2);
+    }
+    if ((threadIdx.x & 31) == 0) { ws[threadIdx.x >> 5] = bs; wi[threadIdx.x >> 5] = bi; }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        bs = ws[threadIdx.x]; bi = wi[threadIdx.x];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            float s2 = __shfl_xor_sync(0xffffffffu, bs, o);
+            int i2 = __shfl_xor_sync(0xffffffffu, bi, o);
+            better(bs, bi, s2, i2);
+        }
+        if (threadIdx.x == 0) a.out_tok[row] = bi;
+    }
+}
+
+int launch_sample(const SampleArgs& a, cudaStream_t st) {
+    if (a.m_max <= 0) return 0;
+    k_sample<<<a.m_max, SMP_THREADS, 0, st>>>(a);
+    return 1;
+}
+
+// grid = n_dump; entry e = (sid, t): if t == *step, find the slot holding sid and copy its row.
+__global__ void k_dump_logits(const int* __restrict__ dump_sid_t, const int* step_dev, const int* __restrict__ live,
+                              const int* n_live, int row_div, const float* __restrict__ logits, int V,
+                              float* __restrict__ out) {
+    __shared__ int slot_s;
+    const int e = blockIdx.x;
+    const int sid = dump_sid_t[2 * e], t = dump_sid_t[2 * e + 1];
+    if (t != *step_dev) return;
+    if (threadIdx.x == 0) slot_s = -1;
+    __syncthreads();
+    const int n = *n_live;
+    for (int i = threadIdx.x; i < n; i += blockDim.x)
+        if (live[i] == sid) slot_s = i;
+    __syncthreads();
+    const int slot = slot_s;
+    if (slot < 0) return;
+    const float* src = logits + (size_t)(slot / row_div) * V;
+    float* dst = out + (size_t)e * V;
+    for (int v = threadIdx.x; v < V; v += blockDim.x) dst[v] = src[v];
+}
+int launch_dump_logits(const int* dump_sid_t, int n_dump, const int* step_dev, const int* live, const int* n_live,
+                       int row_div, const float* logits, int V, float* out, cudaStream_t st) {
+    if (n_dump <= 0) return 0;
+    k_dump_logits<<<n_dump, 256, 0, st>>>(dump_sid_t, step_dev, live, n_live, row_div, logits, V, out);
+    return 1;
+}
+
+}  // namespace sagc

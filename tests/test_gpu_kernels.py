@@ -1,0 +1,147 @@
+"""GPU parity, kernel level: each CUDA kernel reached through the C ABI vs the CPU oracle / fp64 numpy.
+
+Tolerances: integer work bit-exact; advantages 1e-5 relative
+(|a-b| <= 1e-5*max(1,|b|)); projections / attention are compared against fp64 references with
+bounds derived from the arithmetic (bf16 hi+lo activation split: ~2^-16 relative per product).
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import groupstats as ogs
+from oracle import philox as oph
+from oracle import decoder as odec
+from paper_2606_02218_b200 import workloads as wl
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2606_02218_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda()
+
+
+# ---------------------------------------------------------------------------- a14
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("ddof,eps", [(0, 0.0), (1, 1e-6)])
+def test_group_advantage_matches_oracle(B, mode, ddof, eps):
+    rng = np.random.default_rng(7)
+    sizes = list(rng.integers(0, 40, size=200)) + [1, 2, 32, 33, 64, 257, 0]
+    offs = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int32)
+    r = rng.standard_normal(offs[-1]).astype(np.float32)
+    # some all-equal groups, some 0/1 groups, one with a huge offset (cancellation)
+    for g in range(0, 60, 3):
+        r[offs[g]:offs[g + 1]] = np.float32(rng.standard_normal())
+    for g in range(60, 120):
+        r[offs[g]:offs[g + 1]] = (rng.random(sizes[g]) < 0.4).astype(np.float32)
+    r[offs[130]:offs[131]] += np.float32(1e4)
+    adv_o, keep_o = ogs.group_advantage(r, offs, mode, ddof, eps)
+    adv, keep = B.group_advantage(_dev(r), _dev(offs), mode, ddof, eps)
+    assert np.array_equal(keep.cpu().numpy(), keep_o)                     # DAPO mask bit-exact
+    a = adv.cpu().numpy()
+    assert np.all(np.abs(a - adv_o) <= 1e-5 * np.maximum(1.0, np.abs(adv_o)))
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 5])
+def test_group_advantage_on_config_rewards(B, cfg):
+    w = wl.WORKLOADS[cfg]
+    r, offs = wl.make_rewards(w)
+    mode = 1 if w.adv_mode == "DAPO" else 0
+    adv_o, keep_o = ogs.group_advantage(r, offs, mode)
+    adv, keep = B.group_advantage(_dev(r), _dev(offs), mode)
+    assert np.array_equal(keep.cpu().numpy(), keep_o)
+    a = adv.cpu().numpy()
+    assert np.all(np.abs(a - adv_o) <= 1e-5 * np.maximum(1.0, np.abs(adv_o)))
+    for g in range(len(offs) - 1):                                          # invariants on the GPU result
+        seg = a[offs[g]:offs[g + 1]].astype(np.float64)
+        assert abs(seg.sum()) < 1e-4
+        if keep_o[g] and np.ptp(r[offs[g]:offs[g + 1]]) > 0:
+            assert abs(seg.std() - 1.0) < 1e-4
+
+
+def test_group_advantage_empty(B):
+    adv, keep = B.group_advantage(torch.empty(0, dtype=torch.float32, device="cuda"),
+                                  torch.zeros(1, dtype=torch.int32, device="cuda"), 0)
+    assert adv.numel() == 0 and keep.numel() == 0
+
+
+def test_length_stats_bit_exact(B):
+    rng = np.random.default_rng(11)
+    sizes = list(rng.integers(0, 70, size=300)) + [1, 2, 3, 4, 32, 1000]
+    offs = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int32)
+    ell = rng.integers(1, 16385, size=offs[-1]).astype(np.int32)
+    ell[offs[5]:offs[6]] = 77                                             # all equal -> ratio exactly 1
+    st_o, ra_o = ogs.length_stats(ell, offs)
+    st, ra = B.length_stats(_dev(ell), _dev(offs))
+    assert np.array_equal(st.cpu().numpy(), st_o)
+    assert np.array_equal(ra.cpu().numpy().view(np.uint32), ra_o.view(np.uint32))
+    # paper's worked example (tests/golden/length_stats_example.txt)
+    st, ra = B.length_stats(_dev(np.array([100, 200, 300, 1000], np.int32)), _dev(np.array([0, 4], np.int32)))
+    assert st.cpu().numpy().tolist() == [[1000, 1600, 500]] and float(ra[0]) == 2.5
+
+
+# ---------------------------------------------------------------------------- a12
+@pytest.mark.parametrize("seed,sid,t,v0,n", [(0, 0, 1, 0, 64), (4002, 63, 4096, 151900, 36),
+                                             ((0xDEADBEEF << 32) | 0x12345678, 1023, 16384, 5, 1027)])
+def test_philox_draws_bit_exact(B, seed, sid, t, v0, n):
+    got = B.debug_philox(seed, sid, t, v0, n).cpu().numpy().view(np.uint32)
+    assert np.array_equal(got, oph.philox_draws(seed, sid, t, v0, n))
+
+
+# ---------------------------------------------------------------------------- a6, a8-a11
+@pytest.mark.parametrize("N,K", [(64, 128), (896, 896), (896, 4864), (1152, 896), (2048, 1536), (20000 // 16 * 16, 256)])
+@pytest.mark.parametrize("M", [1, 3, 8, 13, 64, 70, 131])
+@pytest.mark.parametrize("path", [1, 2])
+def test_linear_vs_fp64(B, N, K, M, path):
+    if path == 1 and M > 13:
+        pytest.skip("GEMV path is the tail path")
+    rng = np.random.default_rng(N * 31 + K * 7 + M)
+    Wb = wl.f32_to_bf16_bits((0.02 * rng.standard_normal((N, K))).astype(np.float32))
+    x = rng.standard_normal((M, K)).astype(np.float32)
+    ref = x.astype(np.float64) @ wl.bf16_bits_to_f32(Wb).astype(np.float64).T
+    y = B.debug_linear(_dev(Wb.view(np.int16)), _dev(x), path).cpu().numpy()
+    # |err| <= K * 2^-16 * |x||w| (split) + fp32 accumulation; observed ~1e-6.  3e-5 abs is >10x margin.
+    scale = np.sqrt(K) * 0.02
+    assert np.max(np.abs(y - ref)) < 3e-5 * max(1.0, scale), np.max(np.abs(y - ref))
+
+
+# ---------------------------------------------------------------------------- a7
+@pytest.mark.parametrize("Hq,Hkv,hd,page", [(4, 4, 32, 16), (14, 2, 64, 64), (28, 4, 128, 64), (8, 1, 128, 32)])
+def test_paged_attention_vs_fp64(B, Hq, Hkv, hd, page):
+    rng = np.random.default_rng(Hq * 100 + hd)
+    ctxs = np.array([1, 2, page - 1, page, page + 1, 127, 128, 129, 700, 1500], dtype=np.int32)
+    M = len(ctxs)
+    max_blocks = (int(ctxs.max()) + page - 1) // page
+    n_pages = M * max_blocks + 3
+    perm = rng.permutation(n_pages)
+    pt = -np.ones((M, max_blocks), dtype=np.int32)
+    k = 0
+    for m in range(M):
+        for b in range((ctxs[m] + page - 1) // page):
+            pt[m, b] = perm[k]; k += 1
+    kv = wl.f32_to_bf16_bits(rng.standard_normal((n_pages, 2, Hkv, page, hd)).astype(np.float32))
+    kvf = wl.bf16_bits_to_f32(kv).astype(np.float64)
+    q = rng.standard_normal((M, Hq, hd)).astype(np.float32)
+    r = Hq // Hkv
+    ref = np.zeros((M, Hq, hd))
+    for m in range(M):
+        c = int(ctxs[m])
+        K = np.concatenate([kvf[pt[m, b], 0] for b in range((c + page - 1) // page)], axis=1)[:, :c]   # [Hkv][c][hd]
+        V = np.concatenate([kvf[pt[m, b], 1] for b in range((c + page - 1) // page)], axis=1)[:, :c]
+        for h in range(Hq):
+            s = K[h // r] @ q[m, h].astype(np.float64) / np.sqrt(hd)
+            p = np.exp(s - s.max()); p /= p.sum()
+            ref[m, h] = p @ V[h // r]
+    out = B.debug_attention(_dev(q), _dev(kv.view(np.int16)), _dev(pt), _dev(ctxs), Hq, Hkv, hd, page).cpu().numpy()
+    assert np.max(np.abs(out - ref)) < 2e-5, np.max(np.abs(out - ref))
