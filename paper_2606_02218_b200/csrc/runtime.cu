@@ -74,6 +74,8 @@ struct sagc_model {
     int last_nseq, last_max_blocks;
     bool use_pdl;
     int gemv_max;
+    cudaStream_t own_stream;                   // used when the caller passes the legacy default stream
+    cudaEvent_t own_event;
 };
 
 template <typename T>
@@ -99,6 +101,8 @@ static void clear_graphs(sagc_model* m) {
 extern "C" void sagc_model_destroy(sagc_model* m) {
     if (!m) return;
     clear_graphs(m);
+    if (m->own_stream) cudaStreamDestroy(m->own_stream);
+    if (m->own_event) cudaEventDestroy(m->own_event);
     for (void* p : m->allocs) cudaFree(p);
     delete m;
 }
@@ -120,6 +124,7 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
 
     sagc_model* m = new sagc_model();
     m->cfg = c;
+    m->own_stream = nullptr; m->own_event = nullptr;
     const int L = c.n_layers;
     auto cp = [&](std::vector<const bf16_t*>& v, const void* const* src) {
         v.resize(L);
@@ -336,6 +341,17 @@ extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, c
     if (!m || !prompt_offsets || !prm || !out_tokens || !out_lengths) return set_err(SAGC_EINVAL, "null argument");
     const sagc_model_config& c = m->cfg;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    if (st == nullptr || st == cudaStreamLegacy) {
+        // the legacy default stream cannot be captured into a graph: run on an internal stream
+        // ordered after it (the call synchronises before returning, so later work is ordered too)
+        if (!m->own_stream) {
+            CU(cudaStreamCreateWithFlags(&m->own_stream, cudaStreamNonBlocking));
+            CU(cudaEventCreateWithFlags(&m->own_event, cudaEventDisableTiming));
+        }
+        CU(cudaEventRecord(m->own_event, st));
+        CU(cudaStreamWaitEvent(m->own_stream, m->own_event, 0));
+        st = m->own_stream;
+    }
     const int nseq = n_prompts * G;
     const int max_new = prm->max_new_tokens;
     const bool structure_only = (prm->flags & SAGC_FLAG_STRUCTURE_ONLY) != 0;
