@@ -2,7 +2,8 @@
 //
 // One CTA per (activation row, kv head, K-split).  The r = Hq/Hkv query heads that share a kv
 // head are processed together so every K/V byte is read once per (row, kv head).  Contexts are
-// walked through the page table in tiles of 128 tokens:
+// walked through the page table in tiles of 64 tokens, staged in shared memory by a 3-stage
+// cp.async pipeline (K and V rows, padded so that per-token 16-byte reads are conflict-free):
 //   phase 1  thread = token: s[h] = q[h] . k  for the r heads (q pre-scaled, fp32, smem broadcast)
 //   softmax  online (running max / sum per head), warp-shuffle reductions, probabilities in smem
 //   phase 2  thread = (token group, 4 head-dim columns): o[h][:] += p[h][tok] * v[tok][:]
@@ -15,13 +16,32 @@
 namespace sagc {
 
 static constexpr int ATT_THREADS = 128;
-static constexpr int ATT_TILE = 128;
+static constexpr int ATT_TILE = 64;          // tokens per pipeline stage
+static constexpr int ATT_STAGES = 3;
 static constexpr int ATT_MAXR = 8;
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, int src_bytes) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(d), "l"(gsrc), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+template <int HD>
+struct AttSmem {
+    static constexpr int ROWB = HD * 2 + 16;                  // padded row: conflict-free LDS.128 by token
+    static constexpr int STAGE = 2 * ATT_TILE * ROWB;         // K rows then V rows
+    static constexpr int BYTES = ATT_STAGES * STAGE;
+};
 
 template <int HD>
 __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     constexpr int LPR = HD / 4;                 // lanes per V row in phase 2
     constexpr int NG = ATT_THREADS / LPR;       // token groups in phase 2
+    constexpr int ROWB = AttSmem<HD>::ROWB;
+    constexpr int CPR = HD * 2 / 16;            // 16-byte chunks per row
+    extern __shared__ __align__(16) unsigned char kv_s[];
     __shared__ __align__(16) float q_s[ATT_MAXR][HD];
     __shared__ __align__(16) float s_s[ATT_MAXR][ATT_TILE];
     __shared__ float m_s[ATT_MAXR], l_s[ATT_MAXR], sc_s[ATT_MAXR];
@@ -43,7 +63,31 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     cps = ((cps + ATT_TILE - 1) / ATT_TILE) * ATT_TILE;
     const int t_begin = split * cps;
     const int t_end = min(ctx, t_begin + cps);
+    const int n_tiles = t_end > t_begin ? (t_end - t_begin + ATT_TILE - 1) / ATT_TILE : 0;
     const float scale = rsqrtf((float)HD);
+    const size_t head_stride = (size_t)a.page * HD;                 // one (page, K|V, kv head) slab
+
+    // async copy of one tile (K and V rows of 64 tokens) into a stage; rows past t_end are zero-filled
+    auto load_tile = [&](int tile, int stage) {
+        unsigned char* base = kv_s + (size_t)stage * AttSmem<HD>::STAGE;
+        const int t0 = t_begin + tile * ATT_TILE;
+#pragma unroll
+        for (int c = tid; c < ATT_TILE * CPR; c += ATT_THREADS) {
+            const int j = c / CPR, part = c % CPR;
+            const int tok = t0 + j;
+            const bool ok = tok < t_end;
+            const int pg = ok ? pt[tok / a.page] : 0;
+            const bf16_t* kp = a.kv_layer + ((size_t)pg * 2 * a.Hkv + kvh) * head_stride +
+                               (size_t)(ok ? tok % a.page : 0) * HD + part * 8;
+            const bf16_t* vp = kp + (size_t)a.Hkv * head_stride;
+            cp_async16(base + (size_t)j * ROWB + part * 16, kp, ok ? 16 : 0);
+            cp_async16(base + (size_t)(ATT_TILE + j) * ROWB + part * 16, vp, ok ? 16 : 0);
+        }
+    };
+    if (n_tiles > 0) load_tile(0, 0);
+    cp_async_commit();
+    if (n_tiles > 1) load_tile(1, 1);
+    cp_async_commit();
 
     for (int i = tid; i < r * HD; i += ATT_THREADS) {
         int h = i / HD, d = i % HD;
@@ -55,56 +99,59 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     for (int h = 0; h < ATT_MAXR; ++h)
 #pragma unroll
         for (int e = 0; e < 4; ++e) acc[h][e] = 0.f;
-    __syncthreads();
 
-    const size_t head_stride = (size_t)a.page * HD;                 // one (page, K|V, kv head) slab
     const int tg = tid / LPR, dl = tid % LPR;
+    // phase-1 mapping: token = tid % 64, heads h = (tid / 64), +2, +4, ...
+    const int p1_tok = tid & (ATT_TILE - 1), p1_h0 = tid / ATT_TILE;
 
-    for (int t0 = t_begin; t0 < t_end; t0 += ATT_TILE) {
+    for (int tile = 0; tile < n_tiles; ++tile) {
+        cp_async_wait<1>();
+        __syncthreads();                         // tile landed; previous tile's stage is free
+        if (tile + 2 < n_tiles) load_tile(tile + 2, (tile + 2) % ATT_STAGES);
+        cp_async_commit();
+        const unsigned char* base = kv_s + (size_t)(tile % ATT_STAGES) * AttSmem<HD>::STAGE;
+        const int t0 = t_begin + tile * ATT_TILE;
         // ---- phase 1: scores --------------------------------------------------------
         {
-            const int tok = t0 + tid;
-            float s[ATT_MAXR];
+            float s[ATT_MAXR / 2];
 #pragma unroll
-            for (int h = 0; h < ATT_MAXR; ++h) s[h] = 0.f;
-            if (tok < t_end) {
-                const int pg = pt[tok / a.page];
-                const bf16_t* kp = a.kv_layer + ((size_t)pg * 2 * a.Hkv + kvh) * head_stride +
-                                   (size_t)(tok % a.page) * HD;
+            for (int hh = 0; hh < ATT_MAXR / 2; ++hh) s[hh] = 0.f;
+            const unsigned char* kp = base + (size_t)p1_tok * ROWB;
 #pragma unroll 4
-                for (int d = 0; d < HD; d += 8) {
-                    uint4 w = *reinterpret_cast<const uint4*>(kp + d);
-                    float k0 = bf16lo_to_f32(w.x), k1 = bf16hi_to_f32(w.x), k2 = bf16lo_to_f32(w.y),
-                          k3 = bf16hi_to_f32(w.y), k4 = bf16lo_to_f32(w.z), k5 = bf16hi_to_f32(w.z),
-                          k6 = bf16lo_to_f32(w.w), k7 = bf16hi_to_f32(w.w);
+            for (int d = 0; d < HD; d += 8) {
+                uint4 w = *reinterpret_cast<const uint4*>(kp + d * 2);
+                float k0 = bf16lo_to_f32(w.x), k1 = bf16hi_to_f32(w.x), k2 = bf16lo_to_f32(w.y),
+                      k3 = bf16hi_to_f32(w.y), k4 = bf16lo_to_f32(w.z), k5 = bf16hi_to_f32(w.z),
+                      k6 = bf16lo_to_f32(w.w), k7 = bf16hi_to_f32(w.w);
 #pragma unroll
-                    for (int h = 0; h < ATT_MAXR; ++h) {
-                        if (h < r) {
-                            float4 qa = *reinterpret_cast<const float4*>(&q_s[h][d]);
-                            float4 qb = *reinterpret_cast<const float4*>(&q_s[h][d + 4]);
-                            float t = s[h];
-                            t = fmaf(qa.x, k0, t); t = fmaf(qa.y, k1, t); t = fmaf(qa.z, k2, t); t = fmaf(qa.w, k3, t);
-                            t = fmaf(qb.x, k4, t); t = fmaf(qb.y, k5, t); t = fmaf(qb.z, k6, t); t = fmaf(qb.w, k7, t);
-                            s[h] = t;
-                        }
+                for (int hh = 0; hh < ATT_MAXR / 2; ++hh) {
+                    const int h = p1_h0 + 2 * hh;
+                    if (h < r) {
+                        float4 qa = *reinterpret_cast<const float4*>(&q_s[h][d]);
+                        float4 qb = *reinterpret_cast<const float4*>(&q_s[h][d + 4]);
+                        float t = s[hh];
+                        t = fmaf(qa.x, k0, t); t = fmaf(qa.y, k1, t); t = fmaf(qa.z, k2, t); t = fmaf(qa.w, k3, t);
+                        t = fmaf(qb.x, k4, t); t = fmaf(qb.y, k5, t); t = fmaf(qb.z, k6, t); t = fmaf(qb.w, k7, t);
+                        s[hh] = t;
                     }
                 }
             }
 #pragma unroll
-            for (int h = 0; h < ATT_MAXR; ++h)
-                if (h < r) s_s[h][tid] = (tok < t_end) ? s[h] : -INFINITY;
+            for (int hh = 0; hh < ATT_MAXR / 2; ++hh) {
+                const int h = p1_h0 + 2 * hh;
+                if (h < r) s_s[h][p1_tok] = (t0 + p1_tok < t_end) ? s[hh] : -INFINITY;
+            }
         }
         __syncthreads();
         // ---- online softmax: warp w owns heads w, w+4 ----------------------------------
         for (int h = warp; h < r; h += 4) {
-            float4 v = *reinterpret_cast<const float4*>(&s_s[h][lane * 4]);
-            float tmax = warp_max(fmaxf(fmaxf(v.x, v.y), fmaxf(v.z, v.w)));
+            float2 v = *reinterpret_cast<const float2*>(&s_s[h][lane * 2]);
+            float tmax = warp_max(fmaxf(v.x, v.y));
             const float m_old = m_s[h];
             const float m_new = fmaxf(m_old, tmax);
             v.x = __expf(v.x - m_new); v.y = __expf(v.y - m_new);
-            v.z = __expf(v.z - m_new); v.w = __expf(v.w - m_new);
-            *reinterpret_cast<float4*>(&s_s[h][lane * 4]) = v;
-            const float lsum = warp_sum(v.x + v.y + v.z + v.w);
+            *reinterpret_cast<float2*>(&s_s[h][lane * 2]) = v;
+            const float lsum = warp_sum(v.x + v.y);
             if (lane == 0) {
                 const float f = __expf(m_old - m_new);      // exp(-inf) = 0 on the first tile
                 sc_s[h] = f;
@@ -122,14 +169,10 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
                 for (int e = 0; e < 4; ++e) acc[h][e] *= f;
             }
         }
-        const int n_tok = min(ATT_TILE, t_end - t0);
-#pragma unroll 2
-        for (int j = tg; j < n_tok; j += NG) {
-            const int tok = t0 + j;
-            const int pg = pt[tok / a.page];
-            const bf16_t* vp = a.kv_layer + (((size_t)pg * 2 + 1) * a.Hkv + kvh) * head_stride +
-                               (size_t)(tok % a.page) * HD + dl * 4;
-            uint2 w = *reinterpret_cast<const uint2*>(vp);
+        const unsigned char* vbase = base + (size_t)ATT_TILE * ROWB + dl * 8;
+#pragma unroll 4
+        for (int j = tg; j < ATT_TILE; j += NG) {
+            uint2 w = *reinterpret_cast<const uint2*>(vbase + (size_t)j * ROWB);
             const float v0 = bf16lo_to_f32(w.x), v1 = bf16hi_to_f32(w.x), v2 = bf16lo_to_f32(w.y),
                         v3 = bf16hi_to_f32(w.y);
 #pragma unroll
@@ -141,8 +184,9 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
                 }
             }
         }
-        __syncthreads();
     }
+    cp_async_wait<0>();
+    __syncthreads();
 
     // ---- reduce the NG token groups (fixed order) -----------------------------------------
 #pragma unroll
@@ -198,14 +242,25 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     if (tid == 0) a.counters[row * a.Hkv + kvh] = 0;
 }
 
+template <int HD>
+static int launch_att(const AttnArgs& a, cudaStream_t st) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(k_attention<HD>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttSmem<HD>::BYTES) != cudaSuccess)
+            return -1;
+        attr_set = true;
+    }
+    dim3 grid(a.m_max, a.Hkv, a.n_splits);
+    k_attention<HD><<<grid, ATT_THREADS, AttSmem<HD>::BYTES, st>>>(a);
+    return 1;
+}
+
 int launch_attention(const AttnArgs& a, cudaStream_t st) {
     if (a.m_max <= 0) return 0;
-    dim3 grid(a.m_max, a.Hkv, a.n_splits);
-    if (a.hd == 128) k_attention<128><<<grid, ATT_THREADS, 0, st>>>(a);
-    else if (a.hd == 64) k_attention<64><<<grid, ATT_THREADS, 0, st>>>(a);
-    else if (a.hd == 32) k_attention<32><<<grid, ATT_THREADS, 0, st>>>(a);
-    else return -1;
-    return 1;
+    if (a.hd == 128) return launch_att<128>(a, st);
+    if (a.hd == 64) return launch_att<64>(a, st);
+    if (a.hd == 32) return launch_att<32>(a, st);
+    return -1;
 }
 
 }  // namespace sagc

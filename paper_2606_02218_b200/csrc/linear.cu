@@ -363,6 +363,174 @@ __global__ void __launch_bounds__(LIN_THREADS) k_linear_narrow(LinDev a) {
 }
 
 // ---------------------------------------------------------------------------------------
+// tail kernel (M <= 8): no shared-memory staging at all.  Weight fragments AND the matching
+// fp32 activation slices are fetched straight into registers (the activations are a few KB and
+// L2-resident), split hi/lo on the fly and fed to HMMA.  SPLITK: the 8 warps of a CTA share one
+// 16-row tile and interleave the 32-wide k blocks (narrow N); otherwise one tile per warp.
+// ---------------------------------------------------------------------------------------
+template <int EPI, bool SPLITK>
+__global__ void __launch_bounds__(LIN_THREADS) k_linear_tail(LinDev a) {
+    constexpr int NS = (EPI == EPI_SWIGLU) ? 2 : 1;
+    constexpr int U = 4;                                   // k blocks in flight per warp
+    __shared__ float red[SPLITK ? NS * LIN_WARPS * 4 * 32 : 1];
+    __shared__ float ssq_w[LIN_WARPS][8];
+    __shared__ float rstd_s[8];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = lane >> 2, q = lane & 3;
+    const int row0 = (SPLITK ? blockIdx.x : blockIdx.x * LIN_WARPS + warp) * 16;
+    const bool active = row0 < a.N;
+    const int kb0 = SPLITK ? warp : 0, kbs = SPLITK ? LIN_WARPS : 1;
+    const int n_kb = a.K >> 5;
+    const bf16_t* pa[NS]; const bf16_t* pb[NS];
+    if (active) {
+        if (EPI == EPI_SWIGLU) {
+            pa[0] = a.W0 + (size_t)(row0 + g) * a.K + 8 * q;
+            pb[0] = a.W0 + (size_t)(row0 + g + 8) * a.K + 8 * q;
+            pa[NS - 1] = a.W1 + (size_t)(row0 + g) * a.K + 8 * q;
+            pb[NS - 1] = a.W1 + (size_t)(row0 + g + 8) * a.K + 8 * q;
+        } else {
+            pa[0] = seg_row(a, row0 + g) + 8 * q;
+            pb[0] = seg_row(a, row0 + g + 8) + 8 * q;
+        }
+    }
+    uint4 w[NS][U][2];
+    auto load_w = [&](int u, int kb) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            if (active && kb < n_kb) {
+                w[s][u][0] = ldg_stream(pa[s] + (size_t)kb * 32);
+                w[s][u][1] = ldg_stream(pb[s] + (size_t)kb * 32);
+            } else {
+                w[s][u][0] = make_uint4(0, 0, 0, 0);
+                w[s][u][1] = w[s][u][0];
+            }
+        }
+    };
+#pragma unroll
+    for (int u = 0; u < U; ++u) load_w(u, kb0 + u * kbs);
+    pdl_wait();
+    pdl_launch();
+    const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
+    if (M <= 0) return;
+    const float* xrow = a.X + (size_t)g * a.K + 8 * q;
+    const bool xok = g < M;
+    float4 x[U][2];
+    auto load_x = [&](int u, int kb) {
+        if (xok && kb < n_kb) {
+            const float4* p = reinterpret_cast<const float4*>(xrow + (size_t)kb * 32);
+            x[u][0] = __ldcg(p); x[u][1] = __ldcg(p + 1);
+        } else {
+            x[u][0] = make_float4(0.f, 0.f, 0.f, 0.f); x[u][1] = x[u][0];
+        }
+    };
+#pragma unroll
+    for (int u = 0; u < U; ++u) load_x(u, kb0 + u * kbs);
+
+    float acc[NS][4];
+#pragma unroll
+    for (int s = 0; s < NS; ++s)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) acc[s][e] = 0.f;
+    float ssq = 0.f;
+
+    for (int kbase = kb0; kbase < n_kb; kbase += U * kbs) {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int kb = kbase + u * kbs;
+            float4 x0 = x[u][0], x1 = x[u][1];
+            uint4 wa[NS], wb[NS];
+#pragma unroll
+            for (int s = 0; s < NS; ++s) { wa[s] = w[s][u][0]; wb[s] = w[s][u][1]; }
+            // refill this ring slot before the math
+            load_w(u, kb + U * kbs);
+            load_x(u, kb + U * kbs);
+            if (kb < n_kb) {
+                ssq += x0.x * x0.x + x0.y * x0.y + x0.z * x0.z + x0.w * x0.w + x1.x * x1.x + x1.y * x1.y +
+                       x1.z * x1.z + x1.w * x1.w;
+                if (a.norm_w != nullptr) {
+                    uint4 nw = *reinterpret_cast<const uint4*>(a.norm_w + (size_t)kb * 32 + 8 * q);
+                    x0.x *= bf16lo_to_f32(nw.x); x0.y *= bf16hi_to_f32(nw.x);
+                    x0.z *= bf16lo_to_f32(nw.y); x0.w *= bf16hi_to_f32(nw.y);
+                    x1.x *= bf16lo_to_f32(nw.z); x1.y *= bf16hi_to_f32(nw.z);
+                    x1.z *= bf16lo_to_f32(nw.w); x1.w *= bf16hi_to_f32(nw.w);
+                }
+                uint4 hi, lo;
+                split2(x0.x, x0.y, hi.x, lo.x);
+                split2(x0.z, x0.w, hi.y, lo.y);
+                split2(x1.x, x1.y, hi.z, lo.z);
+                split2(x1.z, x1.w, hi.w, lo.w);
+#pragma unroll
+                for (int s = 0; s < NS; ++s) {
+                    mma_bf16_16816(acc[s], wa[s].x, wb[s].x, wa[s].y, wb[s].y, hi.x, hi.y);
+                    mma_bf16_16816(acc[s], wa[s].z, wb[s].z, wa[s].w, wb[s].w, hi.z, hi.w);
+                    mma_bf16_16816(acc[s], wa[s].x, wb[s].x, wa[s].y, wb[s].y, lo.x, lo.y);
+                    mma_bf16_16816(acc[s], wa[s].z, wb[s].z, wa[s].w, wb[s].w, lo.z, lo.w);
+                }
+            }
+        }
+    }
+    // row sums of squares: lanes (g, q = 0..3) hold disjoint k slices of batch row g
+    if (a.norm_w != nullptr) {
+        ssq += __shfl_xor_sync(0xffffffffu, ssq, 1);
+        ssq += __shfl_xor_sync(0xffffffffu, ssq, 2);
+        if (q == 0) ssq_w[warp][g] = ssq;
+    }
+    if (SPLITK) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) red[((s * LIN_WARPS + warp) * 4 + e) * 32 + lane] = acc[s][e];
+    }
+    __syncthreads();
+    if (a.norm_w != nullptr && threadIdx.x < 8) {
+        float t = 0.f;
+        if (SPLITK) {
+#pragma unroll
+            for (int wi = 0; wi < LIN_WARPS; ++wi) t += ssq_w[wi][threadIdx.x];
+        }
+        rstd_s[threadIdx.x] = t;
+    }
+    if (!SPLITK && a.norm_w != nullptr) {
+        // every warp saw the whole of X: its own sums are complete
+        __syncwarp();
+    }
+    __syncthreads();
+    if (SPLITK) {
+        if (warp != 0) return;
+        float r[NS][1][4];
+#pragma unroll
+        for (int s = 0; s < NS; ++s)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                float t = 0.f;
+#pragma unroll
+                for (int wi = 0; wi < LIN_WARPS; ++wi) t += red[((s * LIN_WARPS + wi) * 4 + e) * 32 + lane];
+                r[s][0][e] = t;
+            }
+        float rs[8];
+        if (a.norm_w != nullptr) {
+            // in-warp: lanes 0..7 convert the sums, everyone reads through smem (same warp)
+            if (lane < 8) rstd_s[lane] = rsqrtf(rstd_s[lane] / (float)a.K + a.eps);
+            __syncwarp();
+        }
+        (void)rs;
+        if (active) epilogue<1, EPI>(a, r[0], r[NS - 1], row0, 0, M, rstd_s, lane);
+    } else {
+        float* mine = ssq_w[warp];
+        if (a.norm_w != nullptr) {
+            if (lane < 8) mine[lane] = rsqrtf(mine[lane] / (float)a.K + a.eps);
+            __syncwarp();
+        }
+        float r[NS][1][4];
+#pragma unroll
+        for (int s = 0; s < NS; ++s)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) r[s][0][e] = acc[s][e];
+        if (active) epilogue<1, EPI>(a, r[0], r[NS - 1], row0, 0, M, mine, lane);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
 // LIN_GEMV: fp32-activation GEMV for the straggler tail (M <= 4 per pass, exact fp32 x).
 // One warp = two output rows over the full K; 16-byte weight loads, activations through L1.
 // ---------------------------------------------------------------------------------------
@@ -519,9 +687,13 @@ static cudaError_t launch_epi(const LinearArgs& a, const LinDev& d, cudaStream_t
         if (mb == 2) return launch_cfg(k_linear_gemv<2, EPI>, grid, 0, a.pdl, st, d);
         return launch_cfg(k_linear_gemv<4, EPI>, grid, 0, a.pdl, st, d);
     }
-    int nt = a.m_max <= 8 ? 1 : (a.m_max <= 16 ? 2 : (a.m_max <= 32 ? 4 : 8));
-    const int my = (a.m_max + nt * 8 - 1) / (nt * 8);
     const bool wide = tiles >= 148 * LIN_WARPS;
+    if (a.m_max <= 8) {
+        if (wide) return launch_cfg(k_linear_tail<EPI, false>, dim3((tiles + LIN_WARPS - 1) / LIN_WARPS), 0, a.pdl, st, d);
+        return launch_cfg(k_linear_tail<EPI, true>, dim3(tiles), 0, a.pdl, st, d);
+    }
+    int nt = a.m_max <= 16 ? 2 : (a.m_max <= 32 ? 4 : 8);
+    const int my = (a.m_max + nt * 8 - 1) / (nt * 8);
     if (wide) {
         dim3 grid((tiles + LIN_WARPS - 1) / LIN_WARPS, my);
         int smem = 2 * 4 * nt * 1024 + 64 * 4;

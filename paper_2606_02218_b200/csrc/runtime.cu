@@ -296,7 +296,7 @@ static int round_bucket(int live) {
 static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
     const int ctas = m_bucket * m->cfg.n_kv_heads;
     int want = (2 * 148 + ctas - 1) / ctas;
-    int cap = ctx_bound / 256;
+    int cap = ctx_bound / 128;
     if (cap < 1) cap = 1;
     if (want > cap) want = cap;
     if (want > m->max_splits) want = m->max_splits;
