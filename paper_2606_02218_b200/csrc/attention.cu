@@ -30,22 +30,37 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 
 template <int HD>
 struct AttSmem {
-    static constexpr int ROWB = HD * 2 + 16;                  // padded row: conflict-free LDS.128 by token
+    static constexpr int ROWB = HD * 2;                       // unpadded rows, 16-byte chunks XOR-swizzled
     static constexpr int STAGE = 2 * ATT_TILE * ROWB;         // K rows then V rows
     static constexpr int BYTES = ATT_STAGES * STAGE;
 };
 
+__device__ __forceinline__ void ldmatrix_x4_trans(uint32_t (&r)[4], const void* smem_row) {
+    const uint32_t a = (uint32_t)__cvta_generic_to_shared(smem_row);
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];\n"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+                 : "r"(a));
+}
+
+// Tensor-core formulation (HMMA m16n8k16, fp32 accumulate) with full-precision operands:
+//   A rows g (0..7) carry the bf16 "hi" half of head g's operand and rows g+8 its "lo" half, so
+//     S = q_hi.K + q_lo.K  and  O = p_hi.V + p_lo.V  are each the sum of two accumulator rows that
+//     live in the SAME lane (c0/c1 and c2/c3) -- q and p keep ~16 mantissa bits, K and V are exact.
+//   K^T is the B operand of S; lanes read 16-byte chunks of a token's row (the k order inside each
+//     32-wide block is permuted identically for Q, which costs nothing).
+//   V is the B operand of O through ldmatrix.trans.
+// Each warp owns 16 of the 64 tokens of a tile and keeps its own running (max, sum, O); the four
+// warps are merged once at the end.
 template <int HD>
 __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
-    constexpr int LPR = HD / 4;                 // lanes per V row in phase 2
-    constexpr int NG = ATT_THREADS / LPR;       // token groups in phase 2
     constexpr int ROWB = AttSmem<HD>::ROWB;
     constexpr int CPR = HD * 2 / 16;            // 16-byte chunks per row
-    extern __shared__ __align__(16) unsigned char kv_s[];
-    __shared__ __align__(16) float q_s[ATT_MAXR][HD];
-    __shared__ __align__(16) float s_s[ATT_MAXR][ATT_TILE];
-    __shared__ float m_s[ATT_MAXR], l_s[ATT_MAXR], sc_s[ATT_MAXR];
-    __shared__ __align__(16) float red_s[NG][ATT_MAXR][HD + 4];
+    constexpr int KB = HD / 32;                 // 32-wide d blocks
+    constexpr int NT = HD / 8;                  // output n-tiles
+    extern __shared__ __align__(128) unsigned char kv_s[];
+    __shared__ __align__(16) float o_w[4][ATT_MAXR][HD + 4];
+    __shared__ float m_w[4][ATT_MAXR], l_w[4][ATT_MAXR];
+    __shared__ float m_s[ATT_MAXR], l_s[ATT_MAXR];
     __shared__ int last_s;
 
     pdl_wait();
@@ -55,6 +70,7 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     if (row >= M) return;
     const int r = a.Hq / a.Hkv;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int g = lane >> 2, q = lane & 3;
     const int ctx = a.row_ctx[row];
     const int sid = a.row_sid[row];
     const int* pt = a.page_table + (size_t)sid * a.max_blocks;
@@ -64,10 +80,11 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     const int t_begin = split * cps;
     const int t_end = min(ctx, t_begin + cps);
     const int n_tiles = t_end > t_begin ? (t_end - t_begin + ATT_TILE - 1) / ATT_TILE : 0;
-    const float scale = rsqrtf((float)HD);
     const size_t head_stride = (size_t)a.page * HD;                 // one (page, K|V, kv head) slab
 
-    // async copy of one tile (K and V rows of 64 tokens) into a stage; rows past t_end are zero-filled
+    // K chunk c of token j -> chunk c ^ ksw(j); V chunk c -> c ^ vsw(j)   (bank-conflict free)
+    auto ksw = [](int j) { return CPR >= 8 ? ((j & 1) << 2) : 0; };
+    auto vsw = [](int j) { return CPR >= 8 ? (j & 7) : ((j >> 1) & 3); };
     auto load_tile = [&](int tile, int stage) {
         unsigned char* base = kv_s + (size_t)stage * AttSmem<HD>::STAGE;
         const int t0 = t_begin + tile * ATT_TILE;
@@ -80,8 +97,8 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
             const bf16_t* kp = a.kv_layer + ((size_t)pg * 2 * a.Hkv + kvh) * head_stride +
                                (size_t)(ok ? tok % a.page : 0) * HD + part * 8;
             const bf16_t* vp = kp + (size_t)a.Hkv * head_stride;
-            cp_async16(base + (size_t)j * ROWB + part * 16, kp, ok ? 16 : 0);
-            cp_async16(base + (size_t)(ATT_TILE + j) * ROWB + part * 16, vp, ok ? 16 : 0);
+            cp_async16(base + (size_t)j * ROWB + ((part ^ ksw(j)) << 4), kp, ok ? 16 : 0);
+            cp_async16(base + (size_t)(ATT_TILE + j) * ROWB + ((part ^ vsw(j)) << 4), vp, ok ? 16 : 0);
         }
     };
     if (n_tiles > 0) load_tile(0, 0);
@@ -89,120 +106,130 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     if (n_tiles > 1) load_tile(1, 1);
     cp_async_commit();
 
-    for (int i = tid; i < r * HD; i += ATT_THREADS) {
-        int h = i / HD, d = i % HD;
-        q_s[h][d] = a.q[(size_t)row * a.ldq + (size_t)(kvh * r + h) * HD + d] * scale;
+    // Q fragments (hi in rows g, lo in rows g+8), pre-scaled by 1/sqrt(hd); head g of this kv head
+    uint32_t qf[KB][8];
+    {
+        const float scale = rsqrtf((float)HD);
+        const float* qp = a.q + (size_t)row * a.ldq + (size_t)(kvh * r + g) * HD + 8 * q;
+#pragma unroll
+        for (int kb = 0; kb < KB; ++kb) {
+            float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0;
+            if (g < r) {
+                x0 = *reinterpret_cast<const float4*>(qp + kb * 32);
+                x1 = *reinterpret_cast<const float4*>(qp + kb * 32 + 4);
+            }
+            split2(x0.x * scale, x0.y * scale, qf[kb][0], qf[kb][4]);
+            split2(x0.z * scale, x0.w * scale, qf[kb][1], qf[kb][5]);
+            split2(x1.x * scale, x1.y * scale, qf[kb][2], qf[kb][6]);
+            split2(x1.z * scale, x1.w * scale, qf[kb][3], qf[kb][7]);
+        }
     }
-    if (tid < ATT_MAXR) { m_s[tid] = -INFINITY; l_s[tid] = 0.f; }
-    float acc[ATT_MAXR][4];
+    float o[NT][4];
 #pragma unroll
-    for (int h = 0; h < ATT_MAXR; ++h)
+    for (int n = 0; n < NT; ++n)
 #pragma unroll
-        for (int e = 0; e < 4; ++e) acc[h][e] = 0.f;
-
-    const int tg = tid / LPR, dl = tid % LPR;
-    // phase-1 mapping: token = tid % 64, heads h = (tid / 64), +2, +4, ...
-    const int p1_tok = tid & (ATT_TILE - 1), p1_h0 = tid / ATT_TILE;
+        for (int e = 0; e < 4; ++e) o[n][e] = 0.f;
+    float m_run = -INFINITY, l_run = 0.f;       // head g (replicated over the quad)
 
     for (int tile = 0; tile < n_tiles; ++tile) {
         cp_async_wait<1>();
-        __syncthreads();                         // tile landed; previous tile's stage is free
+        __syncthreads();                         // tile landed; the stage of tile-1 is free
         if (tile + 2 < n_tiles) load_tile(tile + 2, (tile + 2) % ATT_STAGES);
         cp_async_commit();
-        const unsigned char* base = kv_s + (size_t)(tile % ATT_STAGES) * AttSmem<HD>::STAGE;
-        const int t0 = t_begin + tile * ATT_TILE;
-        // ---- phase 1: scores --------------------------------------------------------
-        {
-            float s[ATT_MAXR / 2];
+        const unsigned char* kbase = kv_s + (size_t)(tile % ATT_STAGES) * AttSmem<HD>::STAGE;
+        const unsigned char* vbase = kbase + (size_t)ATT_TILE * ROWB;
+        const int tw = warp * 16;                // this warp's 16 tokens inside the tile
+        const int t0 = t_begin + tile * ATT_TILE + tw;
+        if (t0 >= t_end) continue;               // warp-uniform: nothing but masked tokens
+        // ---- S = Q K^T for two 8-token n-tiles -------------------------------------------
+        float s[2][4];
 #pragma unroll
-            for (int hh = 0; hh < ATT_MAXR / 2; ++hh) s[hh] = 0.f;
-            const unsigned char* kp = base + (size_t)p1_tok * ROWB;
-#pragma unroll 4
-            for (int d = 0; d < HD; d += 8) {
-                uint4 w = *reinterpret_cast<const uint4*>(kp + d * 2);
-                float k0 = bf16lo_to_f32(w.x), k1 = bf16hi_to_f32(w.x), k2 = bf16lo_to_f32(w.y),
-                      k3 = bf16hi_to_f32(w.y), k4 = bf16lo_to_f32(w.z), k5 = bf16hi_to_f32(w.z),
-                      k6 = bf16lo_to_f32(w.w), k7 = bf16hi_to_f32(w.w);
+        for (int n = 0; n < 2; ++n) {
+            s[n][0] = s[n][1] = s[n][2] = s[n][3] = 0.f;
+            const int j = tw + n * 8 + g;        // B column = token
+            const unsigned char* kr = kbase + (size_t)j * ROWB;
 #pragma unroll
-                for (int hh = 0; hh < ATT_MAXR / 2; ++hh) {
-                    const int h = p1_h0 + 2 * hh;
-                    if (h < r) {
-                        float4 qa = *reinterpret_cast<const float4*>(&q_s[h][d]);
-                        float4 qb = *reinterpret_cast<const float4*>(&q_s[h][d + 4]);
-                        float t = s[hh];
-                        t = fmaf(qa.x, k0, t); t = fmaf(qa.y, k1, t); t = fmaf(qa.z, k2, t); t = fmaf(qa.w, k3, t);
-                        t = fmaf(qb.x, k4, t); t = fmaf(qb.y, k5, t); t = fmaf(qb.z, k6, t); t = fmaf(qb.w, k7, t);
-                        s[hh] = t;
-                    }
-                }
-            }
-#pragma unroll
-            for (int hh = 0; hh < ATT_MAXR / 2; ++hh) {
-                const int h = p1_h0 + 2 * hh;
-                if (h < r) s_s[h][p1_tok] = (t0 + p1_tok < t_end) ? s[hh] : -INFINITY;
+            for (int kb = 0; kb < KB; ++kb) {
+                const uint4 w = *reinterpret_cast<const uint4*>(kr + (((kb * 4 + q) ^ ksw(j)) << 4));
+                mma_bf16_16816(s[n], qf[kb][0], qf[kb][4], qf[kb][1], qf[kb][5], w.x, w.y);
+                mma_bf16_16816(s[n], qf[kb][2], qf[kb][6], qf[kb][3], qf[kb][7], w.z, w.w);
             }
         }
-        __syncthreads();
-        // ---- online softmax: warp w owns heads w, w+4 ----------------------------------
-        for (int h = warp; h < r; h += 4) {
-            float2 v = *reinterpret_cast<const float2*>(&s_s[h][lane * 2]);
-            float tmax = warp_max(fmaxf(v.x, v.y));
-            const float m_old = m_s[h];
-            const float m_new = fmaxf(m_old, tmax);
-            v.x = __expf(v.x - m_new); v.y = __expf(v.y - m_new);
-            *reinterpret_cast<float2*>(&s_s[h][lane * 2]) = v;
-            const float lsum = warp_sum(v.x + v.y);
-            if (lane == 0) {
-                const float f = __expf(m_old - m_new);      // exp(-inf) = 0 on the first tile
-                sc_s[h] = f;
-                l_s[h] = l_s[h] * f + lsum;
-                m_s[h] = m_new;
-            }
+        // full-precision score of head g for tokens (n*8 + 2q, +1): hi row + lo row
+        float sc[4];
+        sc[0] = s[0][0] + s[0][2]; sc[1] = s[0][1] + s[0][3];
+        sc[2] = s[1][0] + s[1][2]; sc[3] = s[1][1] + s[1][3];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int tok = t0 + (e >> 1) * 8 + 2 * q + (e & 1);
+            if (tok >= t_end) sc[e] = -INFINITY;
         }
-        __syncthreads();
-        // ---- phase 2: o += p . V -----------------------------------------------------
+        float tmax = fmaxf(fmaxf(sc[0], sc[1]), fmaxf(sc[2], sc[3]));
+        tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 1));
+        tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 2));
+        const float m_new = fmaxf(m_run, tmax);          // finite: token t0 is valid for every head
+        const float f = __expf(m_run - m_new);           // exp(-inf) = 0 on the first tile
+        float p[4];
 #pragma unroll
-        for (int h = 0; h < ATT_MAXR; ++h) {
-            if (h < r) {
-                const float f = sc_s[h];
+        for (int e = 0; e < 4; ++e) p[e] = __expf(sc[e] - m_new);
+        float ls = p[0] + p[1] + p[2] + p[3];
+        ls += __shfl_xor_sync(0xffffffffu, ls, 1);
+        ls += __shfl_xor_sync(0xffffffffu, ls, 2);
+        l_run = l_run * f + ls;
+        m_run = m_new;
 #pragma unroll
-                for (int e = 0; e < 4; ++e) acc[h][e] *= f;
-            }
-        }
-        const unsigned char* vbase = base + (size_t)ATT_TILE * ROWB + dl * 8;
-#pragma unroll 4
-        for (int j = tg; j < ATT_TILE; j += NG) {
-            uint2 w = *reinterpret_cast<const uint2*>(vbase + (size_t)j * ROWB);
-            const float v0 = bf16lo_to_f32(w.x), v1 = bf16hi_to_f32(w.x), v2 = bf16lo_to_f32(w.y),
-                        v3 = bf16hi_to_f32(w.y);
+        for (int n = 0; n < NT; ++n) { o[n][0] *= f; o[n][1] *= f; o[n][2] *= f; o[n][3] *= f; }
+        // P as the A operand: rows g = hi, rows g+8 = lo; k = 16 tokens
+        uint32_t pa[4];
+        split2(p[0], p[1], pa[0], pa[1]);
+        split2(p[2], p[3], pa[2], pa[3]);
+        // ---- O += P V : V^T fragments through ldmatrix.trans ------------------------------
+        // lane -> (matrix = lane/8, row = lane%8): matrices 0,1 = tokens 0-7 / 8-15 of d block 2c,
+        // matrices 2,3 = the same tokens of d block 2c+1
+        const int lm = lane >> 3, lr = lane & 7;
+        const int vtok = tw + (lm & 1) * 8 + lr;
+        const unsigned char* vr = vbase + (size_t)vtok * ROWB;
 #pragma unroll
-            for (int h = 0; h < ATT_MAXR; ++h) {
-                if (h < r) {
-                    const float p = s_s[h][j];
-                    acc[h][0] = fmaf(p, v0, acc[h][0]); acc[h][1] = fmaf(p, v1, acc[h][1]);
-                    acc[h][2] = fmaf(p, v2, acc[h][2]); acc[h][3] = fmaf(p, v3, acc[h][3]);
-                }
-            }
+        for (int c = 0; c < NT / 2; ++c) {
+            uint32_t b[4];
+            const int chunk = 2 * c + (lm >> 1);
+            ldmatrix_x4_trans(b, vr + ((chunk ^ vsw(vtok)) << 4));
+            mma_bf16_16816(o[2 * c], pa[0], pa[1], pa[2], pa[3], b[0], b[1]);
+            mma_bf16_16816(o[2 * c + 1], pa[0], pa[1], pa[2], pa[3], b[2], b[3]);
         }
     }
     cp_async_wait<0>();
-    __syncthreads();
-
-    // ---- reduce the NG token groups (fixed order) -----------------------------------------
+    // ---- merge the four warps (fixed order) ---------------------------------------------------
+    // lane (g, q) holds head g: o[n][0..1] + o[n][2..3] are columns n*8 + 2q, +1
+    if (g < r) {
 #pragma unroll
-    for (int h = 0; h < ATT_MAXR; ++h)
-        if (h < r) *reinterpret_cast<float4*>(&red_s[tg][h][dl * 4]) = make_float4(acc[h][0], acc[h][1], acc[h][2], acc[h][3]);
+        for (int n = 0; n < NT; ++n) {
+            o_w[warp][g][n * 8 + 2 * q] = o[n][0] + o[n][2];
+            o_w[warp][g][n * 8 + 2 * q + 1] = o[n][1] + o[n][3];
+        }
+        if (q == 0) { m_w[warp][g] = m_run; l_w[warp][g] = l_run; }
+    }
+    __syncthreads();
+    if (tid < r) {
+        float mx = fmaxf(fmaxf(m_w[0][tid], m_w[1][tid]), fmaxf(m_w[2][tid], m_w[3][tid]));
+        float l = 0.f;
+#pragma unroll
+        for (int w2 = 0; w2 < 4; ++w2) l += (m_w[w2][tid] == -INFINITY) ? 0.f : __expf(m_w[w2][tid] - mx) * l_w[w2][tid];
+        m_s[tid] = mx; l_s[tid] = l;
+    }
     __syncthreads();
     for (int i = tid; i < r * HD; i += ATT_THREADS) {
         const int h = i / HD, d = i % HD;
-        float o = 0.f;
+        const float mx = m_s[h];
+        float ov = 0.f;
 #pragma unroll
-        for (int g2 = 0; g2 < NG; ++g2) o += red_s[g2][h][d];
+        for (int w2 = 0; w2 < 4; ++w2)
+            ov += (m_w[w2][h] == -INFINITY) ? 0.f : __expf(m_w[w2][h] - mx) * o_w[w2][h][d];
         const int hq = kvh * r + h;
         if (nsp == 1) {
-            a.out[(size_t)row * a.Hq * HD + (size_t)hq * HD + d] = o / l_s[h];
+            a.out[(size_t)row * a.Hq * HD + (size_t)hq * HD + d] = ov / l_s[h];
         } else {
-            a.part_o[(((size_t)row * a.Hq + hq) * nsp + split) * HD + d] = o;
+            a.part_o[(((size_t)row * a.Hq + hq) * nsp + split) * HD + d] = ov;
         }
     }
     if (nsp == 1) return;

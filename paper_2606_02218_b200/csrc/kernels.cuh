@@ -119,4 +119,24 @@ int launch_gather_rows(const float* x, const int* row_idx, int n, int d, float* 
 int launch_dump_logits(const int* dump_sid_t, int n_dump, const int* step_dev, const int* live, const int* n_live,
                        int row_div, const float* logits, int V, float* out, cudaStream_t st);
 
+
+// ---- tcgen05 path (tc_linear.cu) --------------------------------------------------------------
+struct alignas(64) TcMap { unsigned char opaque[128]; };     // mirrors CUtensorMap
+int tc_make_map(TcMap* out, const void* base, long long rows, int K, int box_rows);
+int tc_nb_index(int m_max);                                  // 0..3 -> UMMA N = 32, 64, 128, 256
+struct TcLinearArgs {
+    const TcMap* a[3];          // weight maps (box 64 x 128): {w} | {q, k, v} | {gate, up}
+    int seg_rows[3];
+    const TcMap* b;             // activation map for the chosen N (box 64 x N): pre-split rows
+    int K, N;                   // N = output rows (EPI_SWIGLU: d_ff)
+    const int* m_dev; int m_max;
+    int epi;
+    float* Y; int ldy; const float* R;
+    bf16_t* xs_out; int ld_xs; const bf16_t* norm_next; float* ssq_out;
+    const float* ssq_in; int ssq_in_tiles; int ssq_ld; float eps; int k_norm;
+    bool pdl;
+};
+int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st);
+int launch_split_rows(const float* x, int K, const int* m_dev, int m_max, bf16_t* xs, cudaStream_t st);
+
 }  // namespace sagc

@@ -74,6 +74,7 @@ struct sagc_model {
     int last_nseq, last_max_blocks;
     bool use_pdl;
     int gemv_max;
+    int skip_mask;                             // SAGC_SKIP debug ablation: 1 attention, 2 sampler, 4 linears, 8 rope, 16 lm head
     cudaStream_t own_stream;                   // used when the caller passes the legacy default stream
     cudaEvent_t own_event;
 };
@@ -143,6 +144,7 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     m->layer_stride = m->page_elems * (size_t)c.n_pages;
     m->use_pdl = env_int("SAGC_PDL", 1) != 0;
     m->gemv_max = env_int("SAGC_GEMV_MAX", 0);
+    m->skip_mask = env_int("SAGC_SKIP", 0);
     m->tok_buf = m->len_buf = m->forced_len_d = m->dump_list_d = m->prompt_tok_d = nullptr;
     m->tok_cap = m->forced_cap = m->dump_cap = m->prompt_cap = 0;
     m->row_cap = 0;
@@ -216,6 +218,7 @@ static int enqueue_layers(sagc_model* m, const RowSet& rs, int n_splits, int kin
     const sagc_model_config& c = m->cfg;
     int n = 0, r;
 #define LAUNCH(expr) do { r = (expr); if (r < 0) return -1; n += r; } while (0)
+    const int skip = m->skip_mask;
     LAUNCH(launch_embed(m->embed, rs.tok, rs.m_dev, rs.m_max, c.d_model, m->x, st));
     const int qd = c.n_q_heads * c.head_dim, kvd = c.n_kv_heads * c.head_dim;
     for (int l = 0; l < c.n_layers; ++l) {
@@ -225,14 +228,14 @@ static int enqueue_layers(sagc_model* m, const RowSet& rs, int n_splits, int kin
         a.X = m->x; a.norm_w = m->norm1[l]; a.eps = c.rms_eps; a.Y = m->qkv; a.R = nullptr; a.ldy = m->Nqkv;
         a.K = c.d_model; a.N = m->Nqkv; a.m_dev = rs.m_dev; a.m_max = rs.m_max; a.epi = EPI_STORE; a.kind = kind;
         a.pdl = m->use_pdl;
-        LAUNCH(launch_linear(a, st));
+        if (!(skip & 4)) LAUNCH(launch_linear(a, st));
 
         RopeArgs ra = {};
         ra.qkv = m->qkv; ra.row_sid = rs.sid; ra.row_pos = rs.pos; ra.m_dev = rs.m_dev; ra.m_max = rs.m_max;
         ra.rope_cs = m->rope_cs; ra.kv_layer = m->kv_pool + (size_t)l * m->layer_stride;
         ra.page_table = m->ps.page_table; ra.max_blocks = m->max_blocks; ra.page = c.page_tokens;
         ra.Hq = c.n_q_heads; ra.Hkv = c.n_kv_heads; ra.hd = c.head_dim;
-        LAUNCH(launch_rope_append(ra, st));
+        if (!(skip & 8)) LAUNCH(launch_rope_append(ra, st));
 
         AttnArgs aa = {};
         aa.q = m->qkv; aa.ldq = m->Nqkv; aa.kv_layer = ra.kv_layer; aa.page_table = m->ps.page_table;
@@ -240,26 +243,26 @@ static int enqueue_layers(sagc_model* m, const RowSet& rs, int n_splits, int kin
         aa.Hq = c.n_q_heads; aa.Hkv = c.n_kv_heads; aa.hd = c.head_dim; aa.page = c.page_tokens;
         aa.n_splits = n_splits; aa.part_o = m->part_o; aa.part_ml = m->part_ml; aa.counters = m->counters;
         aa.out = m->att;
-        LAUNCH(launch_attention(aa, st));
+        if (!(skip & 1)) LAUNCH(launch_attention(aa, st));
 
         LinearArgs o = {};
         o.W[0] = m->wo[l]; o.rows[0] = c.d_model; o.X = m->att; o.Y = m->x; o.R = m->x; o.ldy = c.d_model;
         o.K = qd; o.N = c.d_model; o.m_dev = rs.m_dev; o.m_max = rs.m_max; o.epi = EPI_RESID; o.kind = kind;
         o.pdl = m->use_pdl; o.eps = c.rms_eps;
-        LAUNCH(launch_linear(o, st));
+        if (!(skip & 4)) LAUNCH(launch_linear(o, st));
 
         LinearArgs gu = {};
         gu.W[0] = m->wg[l]; gu.W[1] = m->wu[l]; gu.rows[0] = c.d_ff; gu.rows[1] = c.d_ff;
         gu.X = m->x; gu.norm_w = m->norm2[l]; gu.eps = c.rms_eps; gu.Y = m->act; gu.ldy = c.d_ff;
         gu.K = c.d_model; gu.N = c.d_ff; gu.m_dev = rs.m_dev; gu.m_max = rs.m_max; gu.epi = EPI_SWIGLU; gu.kind = kind;
         gu.pdl = m->use_pdl;
-        LAUNCH(launch_linear(gu, st));
+        if (!(skip & 4)) LAUNCH(launch_linear(gu, st));
 
         LinearArgs dn = {};
         dn.W[0] = m->wd[l]; dn.rows[0] = c.d_model; dn.X = m->act; dn.Y = m->x; dn.R = m->x; dn.ldy = c.d_model;
         dn.K = c.d_ff; dn.N = c.d_model; dn.m_dev = rs.m_dev; dn.m_max = rs.m_max; dn.epi = EPI_RESID; dn.kind = kind;
         dn.pdl = m->use_pdl; dn.eps = c.rms_eps;
-        LAUNCH(launch_linear(dn, st));
+        if (!(skip & 4)) LAUNCH(launch_linear(dn, st));
     }
     return n;
 }
@@ -271,6 +274,7 @@ static int enqueue_lm_head(sagc_model* m, const float* xsrc, const int* m_dev, i
     a.W[0] = m->lm_head; a.rows[0] = c.vocab; a.X = xsrc; a.norm_w = m->final_norm; a.eps = c.rms_eps;
     a.Y = m->logits; a.ldy = c.vocab; a.K = c.d_model; a.N = c.vocab; a.m_dev = m_dev; a.m_max = m_max;
     a.epi = EPI_STORE; a.kind = kind; a.pdl = m->use_pdl;
+    if (m->skip_mask & 16) return 0;
     return launch_linear(a, st);
 }
 
@@ -320,7 +324,7 @@ static int enqueue_decode_step(sagc_model* m, const RolloutDev& rd, int m_bucket
     sa.logits = m->logits; sa.V = m->cfg.vocab; sa.row_sid = m->ps.live; sa.step_dev = m->ps.step;
     sa.m_dev = m->ps.n_live; sa.m_max = m_bucket; sa.params = m->sample_params_d; sa.row_div = 1;
     sa.out_tok = m->sampled;
-    n += launch_sample(sa, st);
+    if (!(m->skip_mask & 2)) n += launch_sample(sa, st);
     if (n_dump > 0)
         n += launch_dump_logits(m->dump_list_d, n_dump, m->ps.step, m->ps.live, m->ps.n_live, 1, m->logits,
                                 m->cfg.vocab, dump_out, st);
@@ -727,6 +731,28 @@ extern "C" int sagc_debug_linear(const void* W, const float* x, float* y, int32_
                                  void* stream) {
     if (!W || !x || !y || M < 1 || N % 16 || K % 32) return set_err(SAGC_EINVAL, "need N %% 16 == 0 and K %% 32 == 0");
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    if (path == SAGC_PATH_GEMM && N % 128 == 0 && K % 64 == 0) {
+        // tcgen05 path: pre-split the activations, build the two tensor maps, one launch
+        const int nbi = tc_nb_index(M), NB = 32 << nbi;
+        bf16_t* xs = nullptr;
+        const size_t rows = 2 * (size_t)(((M + NB / 2 - 1) / (NB / 2)) * (NB / 2));
+        CU(cudaMalloc(&xs, rows * K * sizeof(bf16_t)));
+        CU(cudaMemsetAsync(xs, 0, rows * K * sizeof(bf16_t), st));
+        launch_split_rows(x, K, nullptr, M, xs, st);
+        TcMap ma, mb;
+        if (tc_make_map(&ma, W, N, K, 128) != 0 || tc_make_map(&mb, xs, (long long)rows, K, NB) != 0) {
+            cudaFree(xs);
+            return set_err(SAGC_ECUDA, "cuTensorMapEncodeTiled failed");
+        }
+        TcLinearArgs t = {};
+        t.a[0] = &ma; t.seg_rows[0] = N; t.b = &mb; t.K = K; t.N = N; t.m_dev = nullptr; t.m_max = M; t.epi = EPI_STORE;
+        t.Y = y; t.ldy = N; t.pdl = false;
+        int r = launch_linear_tc(t, st);
+        cudaError_t e = cudaStreamSynchronize(st);
+        cudaFree(xs);
+        if (r < 0 || e != cudaSuccess) return set_err(SAGC_ECUDA, "tcgen05 linear: %s", cudaGetErrorString(e != cudaSuccess ? e : cudaGetLastError()));
+        return SAGC_OK;
+    }
     // rows beyond 64 are processed by the kernels' own m-chunk grid dimension
     LinearArgs a = {};
     a.W[0] = reinterpret_cast<const bf16_t*>(W); a.rows[0] = N; a.X = x; a.Y = y; a.ldy = N; a.K = K; a.N = N;

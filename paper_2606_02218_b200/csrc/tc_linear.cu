@@ -1,0 +1,449 @@
+// tc_linear.cu -- tcgen05 / TMEM / TMA projections for the large-batch regime (M > 8 rows) and
+// prefill (steps a2, a6, a8-a11).
+//
+// Swapped-operand skinny GEMM: the bf16 weight tile (128 rows x 64 k, TMA, 128B swizzle) is the
+// UMMA A operand (M = 128); the activations are the B operand.  Activations arrive pre-split in
+// HBM as interleaved bf16 rows  Xs[2m] = hi(x[m]),  Xs[2m+1] = lo(x[m])  (x = hi + lo keeps ~16
+// mantissa bits), so ONE weight tile read from HBM feeds both
+// halves: UMMA N = 2 * (batch rows in the tile), and  y[m][n] = D[n][2m] + D[n][2m+1].
+// fp32 accumulators live in TMEM.  Narrow outputs (N = d_model) are parallelised by splitting K
+// across a thread-block cluster; the partial accumulators are reduced through distributed shared
+// memory in rank order (deterministic), every CTA of the cluster finishing a slice of the batch
+// columns.  Warp roles: 0 = TMA producer, 1 = MMA issuer (one elected lane), 2..5 = epilogue
+// (TMEM lanes 32*(warp%4)); warp 2 also owns the TMEM allocation.
+#include <cooperative_groups.h>
+#include <cuda.h>
+
+#include "common.cuh"
+#include "kernels.cuh"
+
+namespace cg = cooperative_groups;
+
+namespace sagc {
+
+static constexpr int TC_THREADS = 192;
+static constexpr int TC_BK = 64;             // k elements per stage (one 128-byte swizzle atom)
+
+// ---- PTX wrappers ---------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];\n" ::
+            "r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+        : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
+    asm volatile("prefetch.tensormap [%0];\n" ::"l"(map) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+// D[tmem] (+)= A[smem desc] . B[smem desc]^T, bf16 x bf16 -> fp32
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accum) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accum)
+        : "memory");
+}
+// 32 lanes x 32 consecutive fp32 columns: thread t of the warp gets its lane's columns
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, float (&v)[32]) {
+    uint32_t r[32];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, "
+        "%24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+          "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+          "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr));
+    asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+// K-major, 128-byte-swizzled operand tile (rows of 64 bf16 = 128 B, 8-row atoms of 1024 B):
+// start address >> 4 | LBO (unused for swizzled K-major) | SBO = 1024 B | version 1 | SWIZZLE_128B
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr & 0x3ffff) >> 4);
+    d |= (uint64_t)1 << 16;
+    d |= (uint64_t)(1024 >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)2 << 61;
+    return d;
+}
+// kind::f16 instruction descriptor: D = fp32, A = B = bf16, both K-major, M = 128, N = n
+__device__ __forceinline__ uint32_t umma_idesc(int n) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+}
+
+struct TcDev {
+    int K, N;                       // weight shape [N][K]
+    int kb_per_cta;                 // 64-wide k blocks per CTA (cluster rank r takes blocks [r*kb, (r+1)*kb))
+    int n_kb;                       // total k blocks
+    const int* m_dev; int m_max;
+    float* Y; int ldy;              // EPI_STORE / EPI_RESID: fp32 [M][ldy]
+    const float* R;
+    bf16_t* xs_out; int ld_xs;      // EPI_SWIGLU / EPI_RESID: pre-split output rows [2m], [2m+1]
+    const bf16_t* norm_next;        // EPI_RESID: gain of the NEXT RMSNorm, folded into xs_out
+    float* ssq_out;                 // EPI_RESID: [N/128][ssq_ld] partial sums of squares of the new x
+    const float* ssq_in; int ssq_in_tiles;   // fused RMSNorm of the INPUT: rstd[m] from these partials
+    int ssq_ld; float eps; int k_norm;
+};
+
+template <int NB, int NA>
+struct TcCfg {
+    static constexpr int A_BYTES = 128 * 128;
+    static constexpr int B_BYTES = NB * 128;
+    static constexpr int STAGE = NA * A_BYTES + B_BYTES;
+    static constexpr int STAGES = STAGE <= 32 * 1024 ? 6 : (STAGE <= 48 * 1024 ? 4 : 3);
+    static constexpr int MB = NB / 2;
+    static constexpr int TMEM_COLS = NA * NB <= 32 ? 32 : (NA * NB <= 64 ? 64 : (NA * NB <= 128 ? 128 : (NA * NB <= 256 ? 256 : 512)));
+    static constexpr int TAIL = 1024;                                  // barriers, tmem slot, rstd, ssq scratch
+    static constexpr int SMEM = STAGES * STAGE + TAIL + 5 * MB * 4 + 1024;   // + alignment slack
+};
+
+__device__ __forceinline__ float silu_tc(float z) { return z / (1.f + __expf(-z)); }
+
+template <int NB, int EPI>
+__global__ void __launch_bounds__(TC_THREADS, 1)
+k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmA2,
+            const __grid_constant__ CUtensorMap tmA3, const __grid_constant__ CUtensorMap tmB, int seg0, int seg1,
+            TcDev a) {
+    constexpr int NA = (EPI == EPI_SWIGLU) ? 2 : 1;
+    using C = TcCfg<NB, NA>;
+    constexpr int S = C::STAGES, MB = C::MB;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem + S * C::STAGE);
+    uint64_t* empty = full + S;
+    uint64_t* accum = empty + S;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum + 1);
+    float* rstd_s = reinterpret_cast<float*>(smem + S * C::STAGE + C::TAIL);
+    float* ssq_s = rstd_s + MB;                                         // [4][MB]
+    float* red = reinterpret_cast<float*>(smem);                        // [NA][MB][128], overlays the stages
+
+    cg::cluster_group cluster = cg::this_cluster();
+    const int rank = (int)cluster.block_rank();
+    const int KS = (int)cluster.num_blocks();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tile = blockIdx.x, row0 = tile * 128;
+    const int m0 = blockIdx.z * MB;
+    const int kb0 = rank * a.kb_per_cta;
+    const int nk = max(0, min(a.n_kb, kb0 + a.kb_per_cta) - kb0);
+
+    // which weight matrix holds this row tile (q | k | v segments, or gate + up)
+    const CUtensorMap* mapA = &tmA;
+    int arow = row0;
+    if (EPI != EPI_SWIGLU) {
+        if (row0 >= seg1) { mapA = &tmA3; arow = row0 - seg1; }
+        else if (row0 >= seg0) { mapA = &tmA2; arow = row0 - seg0; }
+    }
+
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        mbar_init(accum, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(tmem_slot)),
+                     "n"(C::TMEM_COLS));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            tma_prefetch_desc(mapA);
+            tma_prefetch_desc(&tmB);
+            if (EPI == EPI_SWIGLU) tma_prefetch_desc(&tmA2);
+            // weights never depend on the upstream kernel: fill the ring's A halves before the PDL wait
+            const int pre = min(S, nk);
+            for (int i = 0; i < pre; ++i) {
+                uint8_t* st = smem + i * C::STAGE;
+                mbar_expect_tx(&full[i], C::STAGE);
+                tma_load_2d(st, mapA, &full[i], (kb0 + i) * TC_BK, arow);
+                if (EPI == EPI_SWIGLU) tma_load_2d(st + C::A_BYTES, &tmA2, &full[i], (kb0 + i) * TC_BK, arow);
+            }
+            pdl_wait();
+            for (int i = 0; i < pre; ++i)
+                tma_load_2d(smem + i * C::STAGE + NA * C::A_BYTES, &tmB, &full[i], (kb0 + i) * TC_BK, 2 * m0);
+            for (int i = pre; i < nk; ++i) {
+                const int s = i % S;
+                mbar_wait(&empty[s], ((i / S) - 1) & 1);
+                uint8_t* st = smem + s * C::STAGE;
+                mbar_expect_tx(&full[s], C::STAGE);
+                tma_load_2d(st, mapA, &full[s], (kb0 + i) * TC_BK, arow);
+                if (EPI == EPI_SWIGLU) tma_load_2d(st + C::A_BYTES, &tmA2, &full[s], (kb0 + i) * TC_BK, arow);
+                tma_load_2d(st + NA * C::A_BYTES, &tmB, &full[s], (kb0 + i) * TC_BK, 2 * m0);
+            }
+        }
+        pdl_launch();
+    } else if (warp == 1) {
+        // ===== MMA issuer =====
+        pdl_launch();
+        const uint32_t idesc = umma_idesc(NB);
+        for (int i = 0; i < nk; ++i) {
+            const int s = i % S;
+            mbar_wait(&full[s], (i / S) & 1);
+            tc_fence_after();
+            if (lane == 0) {
+                const uint32_t sa = smem_u32(smem + s * C::STAGE);
+                const uint64_t bdesc = umma_desc_sw128(sa + NA * C::A_BYTES);
+#pragma unroll
+                for (int na = 0; na < NA; ++na) {
+                    const uint64_t adesc = umma_desc_sw128(sa + na * C::A_BYTES);
+#pragma unroll
+                    for (int k = 0; k < TC_BK / 16; ++k)
+                        tc_mma(tmem_base + na * NB, adesc + 2 * k, bdesc + 2 * k, idesc, (i > 0 || k > 0) ? 1u : 0u);
+                }
+                tc_commit(&empty[s]);                 // frees the stage once these MMAs have read it
+                if (i == nk - 1) tc_commit(accum);    // accumulator complete
+            }
+            __syncwarp();
+        }
+    } else {
+        // ===== epilogue warps: TMEM -> (hi + lo) -> shared reduce buffer =====
+        pdl_wait();
+        pdl_launch();
+        const int lg = warp & 3;                      // TMEM lane group of this warp
+        const int row = lg * 32 + lane;
+        const int et = (warp - 2) * 32 + lane;        // 0..127
+        if (a.ssq_in != nullptr) {
+            for (int m = et; m < MB; m += 128) {
+                float t = 0.f;
+                for (int i = 0; i < a.ssq_in_tiles; ++i) t += a.ssq_in[(size_t)i * a.ssq_ld + m0 + m];
+                rstd_s[m] = rsqrtf(t / (float)a.k_norm + a.eps);
+            }
+        }
+        if (nk > 0) {
+            mbar_wait(accum, 0);
+            tc_fence_after();
+        }
+#pragma unroll
+        for (int na = 0; na < NA; ++na) {
+#pragma unroll
+            for (int c = 0; c < NB / 32; ++c) {
+                float v[32];
+                if (nk > 0) {
+                    tc_ld32(tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(na * NB + c * 32), v);
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) v[j] = 0.f;
+                }
+#pragma unroll
+                for (int j = 0; j < 16; ++j) red[((size_t)na * MB + c * 16 + j) * 128 + row] = v[2 * j] + v[2 * j + 1];
+            }
+        }
+        tc_fence_before();
+    }
+    cluster.sync();            // every partial tile of the cluster is in shared memory
+    if (warp >= 2) {
+        const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
+        const int lg = warp & 3;
+        const int row = lg * 32 + lane;
+        const int n = row0 + row;
+        const float* peer[8];
+#pragma unroll
+        for (int p = 0; p < 8; ++p) peer[p] = (p < KS) ? cluster.map_shared_rank(red, p) : red;
+        float nw = 1.f;
+        if (EPI == EPI_RESID && a.norm_next != nullptr) nw = bf16_to_f32(a.norm_next[n]);
+        for (int m = rank; m < MB; m += KS) {
+            const int mg = m0 + m;
+            if (mg >= M) break;
+            float acc[NA];
+#pragma unroll
+            for (int na = 0; na < NA; ++na) {
+                float t = 0.f;
+#pragma unroll
+                for (int p = 0; p < 8; ++p)
+                    if (p < KS) t += peer[p][((size_t)na * MB + m) * 128 + row];
+                acc[na] = t;
+            }
+            const float sc = (a.ssq_in != nullptr) ? rstd_s[m] : 1.f;
+            if (EPI == EPI_STORE) {
+                a.Y[(size_t)mg * a.ldy + n] = acc[0] * sc;
+            } else if (EPI == EPI_RESID) {
+                const size_t o = (size_t)mg * a.ldy + n;
+                const float xn = a.R[o] + acc[0] * sc;
+                a.Y[o] = xn;
+                if (a.xs_out != nullptr) {
+                    const float xw = xn * nw;
+                    const uint32_t hi = f32_to_bf16_bits(xw);
+                    const uint32_t lo = f32_to_bf16_bits(xw - __uint_as_float(hi << 16));
+                    a.xs_out[(size_t)(2 * mg) * a.ld_xs + n] = (bf16_t)hi;
+                    a.xs_out[(size_t)(2 * mg + 1) * a.ld_xs + n] = (bf16_t)lo;
+                }
+                if (a.ssq_out != nullptr) {
+                    const float q2 = warp_sum(xn * xn);
+                    if (lane == 0) ssq_s[lg * MB + m] = q2;
+                }
+            } else {
+                const float v = silu_tc(acc[0] * sc) * (acc[NA - 1] * sc);
+                const uint32_t hi = f32_to_bf16_bits(v);
+                const uint32_t lo = f32_to_bf16_bits(v - __uint_as_float(hi << 16));
+                a.xs_out[(size_t)(2 * mg) * a.ld_xs + n] = (bf16_t)hi;
+                a.xs_out[(size_t)(2 * mg + 1) * a.ld_xs + n] = (bf16_t)lo;
+            }
+        }
+        if (EPI == EPI_RESID && a.ssq_out != nullptr) {
+            asm volatile("bar.sync 1, 128;\n" ::: "memory");
+            const int et = (warp - 2) * 32 + lane;
+            for (int m = et; m < MB; m += 128) {
+                if ((m % KS) == rank && m0 + m < M)
+                    a.ssq_out[(size_t)tile * a.ssq_ld + m0 + m] =
+                        ssq_s[0 * MB + m] + ssq_s[1 * MB + m] + ssq_s[2 * MB + m] + ssq_s[3 * MB + m];
+            }
+        }
+    }
+    tc_fence_before();
+    cluster.sync();            // peers may still be reading this CTA's shared memory
+    if (warp == 2) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "n"(C::TMEM_COLS));
+    }
+}
+
+// ---- x fp32 [M][K] -> pre-split rows (test / debug entry and embedding path) ---------------
+__global__ void k_split_rows(const float* __restrict__ x, int K, const int* m_dev, int m_max, bf16_t* __restrict__ xs) {
+    const int M = m_dev ? min(*m_dev, m_max) : m_max;
+    const int m = blockIdx.x;
+    if (m >= M) return;
+    for (int k = threadIdx.x; k < K; k += blockDim.x) {
+        const float v = x[(size_t)m * K + k];
+        const uint32_t hi = f32_to_bf16_bits(v);
+        xs[(size_t)(2 * m) * K + k] = (bf16_t)hi;
+        xs[(size_t)(2 * m + 1) * K + k] = (bf16_t)f32_to_bf16_bits(v - __uint_as_float(hi << 16));
+    }
+}
+int launch_split_rows(const float* x, int K, const int* m_dev, int m_max, bf16_t* xs, cudaStream_t st) {
+    if (m_max <= 0) return 0;
+    k_split_rows<<<m_max, 256, 0, st>>>(x, K, m_dev, m_max, xs);
+    return 1;
+}
+
+// ---- host: tensor maps ---------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+// bf16 matrix [rows][K] row-major; box = 64 (k) x box_rows, 128-byte swizzle
+int tc_make_map(TcMap* out, const void* base, long long rows, int K, int box_rows) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) return -1;
+    static_assert(sizeof(TcMap) == sizeof(CUtensorMap), "TcMap must mirror CUtensorMap");
+    cuuint64_t dims[2] = {(cuuint64_t)K, (cuuint64_t)rows};
+    cuuint64_t strides[1] = {(cuuint64_t)K * 2};
+    cuuint32_t box[2] = {(cuuint32_t)TC_BK, (cuuint32_t)box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(reinterpret_cast<CUtensorMap*>(out), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims,
+                    strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? 0 : -1;
+}
+
+template <int NB, int EPI>
+static cudaError_t launch_tc_inst(const TcLinearArgs& t, const TcDev& d, dim3 grid, int KS, cudaStream_t st) {
+    constexpr int NA = (EPI == EPI_SWIGLU) ? 2 : 1;
+    const int smem = TcCfg<NB, NA>::SMEM;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(k_linear_tc<NB, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3(TC_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[2];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 1; at[0].val.clusterDim.y = KS; at[0].val.clusterDim.z = 1;
+    at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[1].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = t.pdl ? 2 : 1;
+    const CUtensorMap* a0 = reinterpret_cast<const CUtensorMap*>(t.a[0]);
+    const CUtensorMap* a1 = reinterpret_cast<const CUtensorMap*>(t.a[1] ? t.a[1] : t.a[0]);
+    const CUtensorMap* a2 = reinterpret_cast<const CUtensorMap*>(t.a[2] ? t.a[2] : t.a[0]);
+    const CUtensorMap* b = reinterpret_cast<const CUtensorMap*>(t.b);
+    const int seg0 = t.a[1] ? t.seg_rows[0] : t.N + 128;
+    const int seg1 = t.a[2] ? t.seg_rows[0] + t.seg_rows[1] : t.N + 128;
+    return cudaLaunchKernelEx(&cfg, k_linear_tc<NB, EPI>, *a0, *a1, *a2, *b, seg0, seg1, d);
+}
+
+int tc_nb_index(int m_max) { return m_max <= 16 ? 0 : (m_max <= 32 ? 1 : (m_max <= 64 ? 2 : 3)); }
+
+int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
+    if (t.m_max <= 0) return 0;
+    TcDev d;
+    d.K = t.K; d.N = t.N; d.n_kb = t.K / TC_BK; d.m_dev = t.m_dev; d.m_max = t.m_max; d.Y = t.Y; d.ldy = t.ldy; d.R = t.R;
+    d.xs_out = t.xs_out; d.ld_xs = t.ld_xs; d.norm_next = t.norm_next; d.ssq_out = t.ssq_out; d.ssq_in = t.ssq_in;
+    d.ssq_in_tiles = t.ssq_in_tiles; d.ssq_ld = t.ssq_ld; d.eps = t.eps; d.k_norm = t.k_norm;
+    const int nbi = tc_nb_index(t.m_max);
+    const int NB = 32 << nbi, MB = NB / 2;
+    const int tiles = t.N / 128, mtiles = (t.m_max + MB - 1) / MB;
+    int KS = 148 / (tiles * mtiles);
+    if (KS < 1) KS = 1;
+    if (KS > 8) KS = 8;
+    if (KS > d.n_kb) KS = d.n_kb;
+    d.kb_per_cta = (d.n_kb + KS - 1) / KS;
+    KS = (d.n_kb + d.kb_per_cta - 1) / d.kb_per_cta;
+    dim3 grid(tiles, KS, mtiles);
+    cudaError_t e;
+#define TC_CASE(NBV)                                                                         \
+    case NBV:                                                                                \
+        if (t.epi == EPI_SWIGLU) e = launch_tc_inst<NBV, EPI_SWIGLU>(t, d, grid, KS, st);    \
+        else if (t.epi == EPI_RESID) e = launch_tc_inst<NBV, EPI_RESID>(t, d, grid, KS, st); \
+        else e = launch_tc_inst<NBV, EPI_STORE>(t, d, grid, KS, st);                         \
+        break;
+    switch (NB) {
+        TC_CASE(32)
+        TC_CASE(64)
+        TC_CASE(128)
+        default:
+        TC_CASE(256)
+    }
+#undef TC_CASE
+    return e == cudaSuccess ? 1 : -1;
+}
+
+}  // namespace sagc
