@@ -28,6 +28,17 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
+// attention output element (row, col): fp32, or pre-split hi / lo bf16 rows for the tcgen05 O-projection
+__device__ __forceinline__ void store_out(const AttnArgs& a, int row, int col, float v) {
+    if (a.out_split != nullptr) {
+        const uint32_t hi = f32_to_bf16_bits(v);
+        a.out_split[(size_t)(2 * row) * a.ld_split + col] = (bf16_t)hi;
+        a.out_split[(size_t)(2 * row + 1) * a.ld_split + col] = (bf16_t)f32_to_bf16_bits(v - __uint_as_float(hi << 16));
+    } else {
+        a.out[(size_t)row * a.Hq * a.hd + col] = v;
+    }
+}
+
 template <int HD>
 struct AttSmem {
     static constexpr int ROWB = HD * 2;                       // unpadded rows, 16-byte chunks XOR-swizzled
@@ -227,7 +238,7 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
             ov += (m_w[w2][h] == -INFINITY) ? 0.f : __expf(m_w[w2][h] - mx) * o_w[w2][h][d];
         const int hq = kvh * r + h;
         if (nsp == 1) {
-            a.out[(size_t)row * a.Hq * HD + (size_t)hq * HD + d] = ov / l_s[h];
+            store_out(a, row, hq * HD + d, ov / l_s[h]);
         } else {
             a.part_o[(((size_t)row * a.Hq + hq) * nsp + split) * HD + d] = ov;
         }
@@ -264,7 +275,7 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
                 den += f * l2;
             }
         }
-        a.out[(size_t)row * a.Hq * HD + (size_t)hq * HD + d] = num / den;
+        store_out(a, row, hq * HD + d, num / den);
     }
     if (tid == 0) a.counters[row * a.Hkv + kvh] = 0;
 }

@@ -115,4 +115,45 @@ int launch_prefill_rows(const int* prompt_tokens, const int* prompt_offsets_dev,
     return 1;
 }
 
+// tcgen05 variant of the embedding step: besides the fp32 residual row it writes the pre-split
+// operand rows of the first RMSNorm (x * w_norm as hi / lo bf16) and the row's sum of squares
+// (tile 0 of the partial-sum buffer; the other tiles are zeroed).
+__global__ void __launch_bounds__(256) k_embed_split(const bf16_t* __restrict__ embed, const int* __restrict__ tok,
+                                                     const int* m_dev, int m_max, int d, float* __restrict__ x,
+                                                     const bf16_t* __restrict__ norm_w, bf16_t* __restrict__ xs,
+                                                     float* __restrict__ ssq, int ssq_ld, int ssq_tiles) {
+    __shared__ float red[8];
+    pdl_wait();
+    pdl_launch();
+    const int M = m_dev ? min(*m_dev, m_max) : m_max;
+    const int row = blockIdx.x;
+    if (row >= M) return;
+    const bf16_t* src = embed + (size_t)tok[row] * d;
+    float acc = 0.f;
+    for (int k = threadIdx.x; k < d; k += blockDim.x) {
+        const float v = bf16_to_f32(src[k]);
+        x[(size_t)row * d + k] = v;
+        acc += v * v;
+        const float xw = v * bf16_to_f32(norm_w[k]);
+        const uint32_t hi = f32_to_bf16_bits(xw);
+        xs[(size_t)(2 * row) * d + k] = (bf16_t)hi;
+        xs[(size_t)(2 * row + 1) * d + k] = (bf16_t)f32_to_bf16_bits(xw - __uint_as_float(hi << 16));
+    }
+    acc = warp_sum(acc);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float t = 0.f;
+        for (int i = 0; i < 8; ++i) t += red[i];
+        ssq[row] = t;
+        for (int i = 1; i < ssq_tiles; ++i) ssq[(size_t)i * ssq_ld + row] = 0.f;
+    }
+}
+int launch_embed_split(const bf16_t* embed, const int* tok, const int* m_dev, int m_max, int d, float* x,
+                       const bf16_t* norm_w, bf16_t* xs, float* ssq, int ssq_ld, int ssq_tiles, cudaStream_t st) {
+    if (m_max <= 0) return 0;
+    k_embed_split<<<m_max, 256, 0, st>>>(embed, tok, m_dev, m_max, d, x, norm_w, xs, ssq, ssq_ld, ssq_tiles);
+    return 1;
+}
+
 }  // namespace sagc

@@ -9,7 +9,7 @@ namespace sagc {
 typedef uint16_t bf16_t;   // raw bf16 bit pattern
 
 enum { EPI_STORE = 0, EPI_RESID = 1, EPI_SWIGLU = 2 };
-enum { LIN_MMA = 0, LIN_GEMV = 1 };
+enum { LIN_MMA = 0, LIN_GEMV = 1, LIN_TC = 2 };
 
 // Y[M][N] = epi( rms?(X)[M][K] . W[N][K]^T ).  Steps a6, a8-a11 of DESIGN.md.
 struct LinearArgs {
@@ -61,7 +61,9 @@ struct AttnArgs {
     float* part_o;          // [M][Hq][n_splits][hd] scratch
     float* part_ml;         // [M][Hq][n_splits][2]  (max, sum)
     int* counters;          // [M*Hkv] arrival counters (zero on entry, reset on exit)
-    float* out;             // [M][Hq*hd]
+    float* out;             // [M][Hq*hd] fp32 (used when out_split is null)
+    bf16_t* out_split;      // pre-split rows [2m] = hi, [2m+1] = lo, row stride ld_split (tcgen05 path)
+    int ld_split;
 };
 int launch_attention(const AttnArgs& a, cudaStream_t st);
 
@@ -137,6 +139,8 @@ struct TcLinearArgs {
     bool pdl;
 };
 int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st);
+int launch_embed_split(const bf16_t* embed, const int* tok, const int* m_dev, int m_max, int d, float* x,
+                       const bf16_t* norm_w, bf16_t* xs, float* ssq, int ssq_ld, int ssq_tiles, cudaStream_t st);
 int launch_split_rows(const float* x, int K, const int* m_dev, int m_max, bf16_t* xs, cudaStream_t st);
 
 }  // namespace sagc

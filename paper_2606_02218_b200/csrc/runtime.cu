@@ -75,6 +75,13 @@ struct sagc_model {
     bool use_pdl;
     int gemv_max;
     int skip_mask;                             // SAGC_SKIP debug ablation: 1 attention, 2 sampler, 4 linears, 8 rope, 16 lm head
+    // tcgen05 path: pre-split activation buffers, partial sums of squares, tensor maps
+    bool tc_ok;
+    bf16_t *xs, *att_s, *act_s;
+    float* ssq;
+    int ssq_ld, d_tiles;
+    std::vector<TcMap> wmaps;                  // per layer: q k v o g u d ; last = lm_head
+    TcMap amaps[3][4];                         // {xs, att_s, act_s} x UMMA N {32, 64, 128, 256}
     cudaStream_t own_stream;                   // used when the caller passes the legacy default stream
     cudaEvent_t own_event;
 };
@@ -194,6 +201,39 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     DA(m->offs_d, c.max_seqs + 1);
     DA(m->sample_params_d, 4);
     m->last_nseq = 0; m->last_max_blocks = m->max_blocks;
+    {
+        const int qd = c.n_q_heads * c.head_dim, kvd = c.n_kv_heads * c.head_dim;
+        m->tc_ok = env_int("SAGC_TC", 1) != 0 && L > 0 && c.d_model % 128 == 0 && qd % 128 == 0 && kvd % 128 == 0 &&
+                   c.d_ff % 128 == 0 && c.vocab % 128 == 0;
+        m->xs = m->att_s = m->act_s = nullptr; m->ssq = nullptr;
+        if (m->tc_ok) {
+            const size_t Rp = ((R + 127) / 128) * 128;
+            m->ssq_ld = (int)Rp; m->d_tiles = c.d_model / 128;
+            DA(m->xs, 2 * Rp * c.d_model); DA(m->att_s, 2 * Rp * qd); DA(m->act_s, 2 * Rp * c.d_ff);
+            DA(m->ssq, (size_t)m->d_tiles * Rp);
+            cudaMemset(m->xs, 0, 2 * Rp * c.d_model * 2); cudaMemset(m->att_s, 0, 2 * Rp * qd * 2);
+            cudaMemset(m->act_s, 0, 2 * Rp * c.d_ff * 2); cudaMemset(m->ssq, 0, (size_t)m->d_tiles * Rp * 4);
+            m->wmaps.resize((size_t)L * 7 + 1);
+            int bad = 0;
+            for (int l = 0; l < L; ++l) {
+                TcMap* w7 = &m->wmaps[(size_t)l * 7];
+                bad |= tc_make_map(&w7[0], m->wq[l], qd, c.d_model, 128);
+                bad |= tc_make_map(&w7[1], m->wk[l], kvd, c.d_model, 128);
+                bad |= tc_make_map(&w7[2], m->wv[l], kvd, c.d_model, 128);
+                bad |= tc_make_map(&w7[3], m->wo[l], c.d_model, qd, 128);
+                bad |= tc_make_map(&w7[4], m->wg[l], c.d_ff, c.d_model, 128);
+                bad |= tc_make_map(&w7[5], m->wu[l], c.d_ff, c.d_model, 128);
+                bad |= tc_make_map(&w7[6], m->wd[l], c.d_model, c.d_ff, 128);
+            }
+            bad |= tc_make_map(&m->wmaps[(size_t)L * 7], m->lm_head, c.vocab, c.d_model, 128);
+            for (int i = 0; i < 4; ++i) {
+                bad |= tc_make_map(&m->amaps[0][i], m->xs, 2 * (long long)Rp, c.d_model, 32 << i);
+                bad |= tc_make_map(&m->amaps[1][i], m->att_s, 2 * (long long)Rp, qd, 32 << i);
+                bad |= tc_make_map(&m->amaps[2][i], m->act_s, 2 * (long long)Rp, c.d_ff, 32 << i);
+            }
+            if (bad) { sagc_model_destroy(m); return set_err(SAGC_ECUDA, "cuTensorMapEncodeTiled failed"); }
+        }
+    }
     cudaError_t e = cudaDeviceSynchronize();
     if (e != cudaSuccess) { sagc_model_destroy(m); return set_err(SAGC_ECUDA, "create: %s", cudaGetErrorString(e)); }
     *out = m;
@@ -209,13 +249,18 @@ struct RowSet {
 
 static int pick_kind(const sagc_model* m, int path, int m_max) {
     if (path == SAGC_PATH_GEMV) return LIN_GEMV;
-    if (path == SAGC_PATH_GEMM) return LIN_MMA;
-    return (m_max <= m->gemv_max) ? LIN_GEMV : LIN_MMA;
+    if (path == SAGC_PATH_GEMM) return m->tc_ok ? LIN_TC : LIN_MMA;
+    if (m_max <= m->gemv_max) return LIN_GEMV;
+    if (m_max <= 8 || !m->tc_ok) return LIN_MMA;      // tail: register-resident HMMA kernel
+    return LIN_TC;                                    // large batch / prefill: tcgen05 + TMEM
 }
+
+static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cudaStream_t st);
 
 // layers only (x ends up holding the final residual stream).  Returns kernels launched or <0.
 static int enqueue_layers(sagc_model* m, const RowSet& rs, int n_splits, int kind, cudaStream_t st) {
     const sagc_model_config& c = m->cfg;
+    if (kind == LIN_TC) return enqueue_layers_tc(m, rs, n_splits, st);
     int n = 0, r;
 #define LAUNCH(expr) do { r = (expr); if (r < 0) return -1; n += r; } while (0)
     const int skip = m->skip_mask;
@@ -267,14 +312,83 @@ static int enqueue_layers(sagc_model* m, const RowSet& rs, int n_splits, int kin
     return n;
 }
 
+// tcgen05 variant of the layer stack: activations travel between kernels as pre-split bf16 rows
+// (xs / att_s / act_s), the RMSNorm gain is folded in by the producer and 1/rms by the consumer.
+static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cudaStream_t st) {
+    const sagc_model_config& c = m->cfg;
+    int n = 0, r;
+    const int skip = m->skip_mask;
+    const int qd = c.n_q_heads * c.head_dim, kvd = c.n_kv_heads * c.head_dim;
+    const int nbi = tc_nb_index(rs.m_max);
+    LAUNCH(launch_embed_split(m->embed, rs.tok, rs.m_dev, rs.m_max, c.d_model, m->x, m->norm1[0], m->xs, m->ssq,
+                              m->ssq_ld, m->d_tiles, st));
+    for (int l = 0; l < c.n_layers; ++l) {
+        const TcMap* w7 = &m->wmaps[(size_t)l * 7];
+        TcLinearArgs t = {};
+        t.a[0] = &w7[0]; t.a[1] = &w7[1]; t.a[2] = &w7[2]; t.seg_rows[0] = qd; t.seg_rows[1] = kvd; t.seg_rows[2] = kvd;
+        t.b = &m->amaps[0][nbi]; t.K = c.d_model; t.N = m->Nqkv; t.m_dev = rs.m_dev; t.m_max = rs.m_max; t.epi = EPI_STORE;
+        t.Y = m->qkv; t.ldy = m->Nqkv; t.ssq_in = m->ssq; t.ssq_in_tiles = m->d_tiles; t.ssq_ld = m->ssq_ld;
+        t.eps = c.rms_eps; t.k_norm = c.d_model; t.pdl = m->use_pdl;
+        if (!(skip & 4)) LAUNCH(launch_linear_tc(t, st));
+
+        RopeArgs ra = {};
+        ra.qkv = m->qkv; ra.row_sid = rs.sid; ra.row_pos = rs.pos; ra.m_dev = rs.m_dev; ra.m_max = rs.m_max;
+        ra.rope_cs = m->rope_cs; ra.kv_layer = m->kv_pool + (size_t)l * m->layer_stride;
+        ra.page_table = m->ps.page_table; ra.max_blocks = m->max_blocks; ra.page = c.page_tokens;
+        ra.Hq = c.n_q_heads; ra.Hkv = c.n_kv_heads; ra.hd = c.head_dim;
+        if (!(skip & 8)) LAUNCH(launch_rope_append(ra, st));
+
+        AttnArgs aa = {};
+        aa.q = m->qkv; aa.ldq = m->Nqkv; aa.kv_layer = ra.kv_layer; aa.page_table = m->ps.page_table;
+        aa.max_blocks = m->max_blocks; aa.row_sid = rs.sid; aa.row_ctx = rs.ctx; aa.m_dev = rs.m_dev; aa.m_max = rs.m_max;
+        aa.Hq = c.n_q_heads; aa.Hkv = c.n_kv_heads; aa.hd = c.head_dim; aa.page = c.page_tokens;
+        aa.n_splits = n_splits; aa.part_o = m->part_o; aa.part_ml = m->part_ml; aa.counters = m->counters;
+        aa.out = m->att; aa.out_split = m->att_s; aa.ld_split = qd;
+        if (!(skip & 1)) LAUNCH(launch_attention(aa, st));
+
+        TcLinearArgs o = {};
+        o.a[0] = &w7[3]; o.seg_rows[0] = c.d_model; o.b = &m->amaps[1][nbi]; o.K = qd; o.N = c.d_model;
+        o.m_dev = rs.m_dev; o.m_max = rs.m_max; o.epi = EPI_RESID; o.Y = m->x; o.R = m->x; o.ldy = c.d_model;
+        o.xs_out = m->xs; o.ld_xs = c.d_model; o.norm_next = m->norm2[l]; o.ssq_out = m->ssq; o.ssq_ld = m->ssq_ld;
+        o.eps = c.rms_eps; o.pdl = m->use_pdl;
+        if (!(skip & 4)) LAUNCH(launch_linear_tc(o, st));
+
+        TcLinearArgs gu = {};
+        gu.a[0] = &w7[4]; gu.a[1] = &w7[5]; gu.seg_rows[0] = c.d_ff; gu.seg_rows[1] = c.d_ff;
+        gu.b = &m->amaps[0][nbi]; gu.K = c.d_model; gu.N = c.d_ff; gu.m_dev = rs.m_dev; gu.m_max = rs.m_max;
+        gu.epi = EPI_SWIGLU; gu.xs_out = m->act_s; gu.ld_xs = c.d_ff; gu.ssq_in = m->ssq; gu.ssq_in_tiles = m->d_tiles;
+        gu.ssq_ld = m->ssq_ld; gu.eps = c.rms_eps; gu.k_norm = c.d_model; gu.pdl = m->use_pdl;
+        if (!(skip & 4)) LAUNCH(launch_linear_tc(gu, st));
+
+        TcLinearArgs dn = {};
+        dn.a[0] = &w7[6]; dn.seg_rows[0] = c.d_model; dn.b = &m->amaps[2][nbi]; dn.K = c.d_ff; dn.N = c.d_model;
+        dn.m_dev = rs.m_dev; dn.m_max = rs.m_max; dn.epi = EPI_RESID; dn.Y = m->x; dn.R = m->x; dn.ldy = c.d_model;
+        dn.xs_out = m->xs; dn.ld_xs = c.d_model; dn.norm_next = (l + 1 < c.n_layers) ? m->norm1[l + 1] : m->final_norm;
+        dn.ssq_out = m->ssq; dn.ssq_ld = m->ssq_ld; dn.eps = c.rms_eps; dn.pdl = m->use_pdl;
+        if (!(skip & 4)) LAUNCH(launch_linear_tc(dn, st));
+    }
+    return n;
+}
+#undef LAUNCH
+
 // final norm + LM head over rows of `xsrc` -> m->logits
 static int enqueue_lm_head(sagc_model* m, const float* xsrc, const int* m_dev, int m_max, int kind, cudaStream_t st) {
     const sagc_model_config& c = m->cfg;
+    if (m->skip_mask & 16) return 0;
+    if (kind == LIN_TC && xsrc == m->x) {
+        // decode: the last down-projection left x * w_final pre-split in xs and its row sums in ssq
+        TcLinearArgs t = {};
+        t.a[0] = &m->wmaps[(size_t)c.n_layers * 7]; t.seg_rows[0] = c.vocab; t.b = &m->amaps[0][tc_nb_index(m_max)];
+        t.K = c.d_model; t.N = c.vocab; t.m_dev = m_dev; t.m_max = m_max; t.epi = EPI_STORE; t.Y = m->logits; t.ldy = c.vocab;
+        t.ssq_in = m->ssq; t.ssq_in_tiles = m->d_tiles; t.ssq_ld = m->ssq_ld; t.eps = c.rms_eps; t.k_norm = c.d_model;
+        t.pdl = m->use_pdl;
+        return launch_linear_tc(t, st);
+    }
+    if (kind == LIN_TC) kind = LIN_MMA;          // gathered fp32 rows (first token): register HMMA path
     LinearArgs a = {};
     a.W[0] = m->lm_head; a.rows[0] = c.vocab; a.X = xsrc; a.norm_w = m->final_norm; a.eps = c.rms_eps;
     a.Y = m->logits; a.ldy = c.vocab; a.K = c.d_model; a.N = c.vocab; a.m_dev = m_dev; a.m_max = m_max;
     a.epi = EPI_STORE; a.kind = kind; a.pdl = m->use_pdl;
-    if (m->skip_mask & 16) return 0;
     return launch_linear(a, st);
 }
 

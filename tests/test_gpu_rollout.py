@@ -227,3 +227,50 @@ def test_bad_arguments_fail_loudly(B):
     with pytest.raises(B.SagcError):
         m.rollout_group(prompts, offs, 4, mode=B.MODE_GUMBEL, temperature=0.0, max_new_tokens=8)
     m.close()
+
+
+# ---------------------------------------------------------------------------- configs 2..5: sampled slices
+def _sampled_parity(B, cfg, n_prompts, P, G, max_new, fl, path, n_dump_seq=3):
+    """Run a truncated instance of a BASELINE config (full-size model, fewer / shorter sequences) and
+    compare against the oracle teacher-forced on the GPU's own tokens."""
+    w = wl.WORKLOADS[cfg]
+    weights = wl.make_weights(w.model, 0)
+    prompts, offs = wl.make_prompts(w, n_prompts=n_prompts, prompt_len=P)
+    mode = 1 if w.sampling == "gumbel" else 0
+    n_pages = _pool_pages(w, G, n_prompts, P, max_new)
+    m = B.Model(w.model, weights, n_pages, n_prompts * G, P + max_new)
+    sids = list(range(0, n_prompts * G, max(1, (n_prompts * G) // n_dump_seq)))[:n_dump_seq]
+    dump = [(sid, t) for sid in sids for t in sorted({1, 2, int(fl[sid]) // 2 + 1, int(fl[sid])}) if 1 <= t <= fl[sid]]
+    out = m.rollout_group(prompts, offs, G, mode=mode, temperature=w.temperature, seed=w.philox_seed,
+                          max_new_tokens=max_new, forced_lengths=fl, path=path, flags=B.FLAG_LOG, dump=dump)
+    toks = out.tokens.cpu().numpy()
+    lens = out.lengths.cpu().numpy()
+    assert np.array_equal(lens, np.minimum(fl, max_new))
+    st, _ = opg.run_structure_only(n_pages, w.model.page_tokens, [P] * n_prompts, G, fl, max_new)
+    _check_structure(B, m, st, out, lens)
+    dec = odec.RefDecoder(w.model, weights)
+    lg = out.dump_logits.cpu().numpy()
+    worst, n_bad, n_dis, n_all = 0.0, 0, 0, 0
+    for sid in sids:
+        p = sid // G
+        steps = [t for (s, t) in dump if s == sid]
+        ref = oro.teacher_forced_logits(dec, prompts[offs[p]:offs[p + 1]], toks[sid, :lens[sid]], steps)
+        for i, t in enumerate(steps):
+            k = dump.index((sid, t))
+            worst = max(worst, float(np.max(np.abs(lg[k] - ref[i]))))
+            s = oph.perturbed_scores(ref[i], mode, w.temperature, w.philox_seed, sid, t)
+            n_all += 1
+            if int(np.argmax(s)) != int(toks[sid, t - 1]):
+                n_dis += 1
+                n_bad += oph.top2_margin(s) >= 1e-2
+    m.close()
+    assert worst <= 3e-2, worst
+    assert n_bad == 0, (n_bad, n_dis, n_all)
+    return worst
+
+
+@pytest.mark.parametrize("path", [0, 2])
+def test_config2_truncated(B, path):
+    """0.5B shape: 2 prompts x 256 x G=8 (16 live -> tcgen05 path, then the tail path below 9 live)."""
+    fl = np.array([3, 14, 14, 2, 14, 9, 5, 14, 14, 1, 14, 7, 14, 14, 4, 14], dtype=np.int32)
+    _sampled_parity(B, 2, 2, 256, 8, 14, fl, path)
