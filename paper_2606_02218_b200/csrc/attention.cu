@@ -19,6 +19,7 @@ static constexpr int ATT_THREADS = 128;
 static constexpr int ATT_TILE = 64;          // tokens per pipeline stage
 static constexpr int ATT_STAGES = 3;
 static constexpr int ATT_MAXR = 8;
+static constexpr int ATT_MAXPG = 1104;       // page ids cached per split (17408 / 16 + slack)
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, int src_bytes) {
     const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
@@ -74,11 +75,16 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     __shared__ float m_s[ATT_MAXR], l_s[ATT_MAXR];
     __shared__ int last_s;
 
-    pdl_wait();
-    pdl_launch();
+    __shared__ int pg_s[ATT_MAXPG];               // page ids of this split's blocks
+    trace_mark(12);
+    // Decode (a.prefetch): the live list, contexts, page table and every cached position but the
+    // newest were written by EARLIER steps, so they may be read before the upstream kernel (this
+    // step's RoPE / KV append) has finished.  Prefill rows attend to positions appended by that very
+    // kernel and must wait first.
+    if (!a.prefetch) pdl_wait();
     const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
     const int row = blockIdx.x, kvh = blockIdx.y, split = blockIdx.z;
-    if (row >= M) return;
+    if (row >= M) { if (a.prefetch) pdl_wait(); pdl_launch(); return; }
     const int r = a.Hq / a.Hkv;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g = lane >> 2, q = lane & 3;
@@ -92,6 +98,14 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     const int t_end = min(ctx, t_begin + cps);
     const int n_tiles = t_end > t_begin ? (t_end - t_begin + ATT_TILE - 1) / ATT_TILE : 0;
     const size_t head_stride = (size_t)a.page * HD;                 // one (page, K|V, kv head) slab
+    const int pshift = 31 - __clz(a.page), pmask = a.page - 1;      // page_tokens is a power of two
+    const int b_begin = t_begin >> pshift;
+    const int n_blk = t_end > t_begin ? ((t_end - 1) >> pshift) - b_begin + 1 : 0;
+    const bool pg_cached = n_blk <= ATT_MAXPG;
+    if (pg_cached) {
+        for (int b = tid; b < n_blk; b += ATT_THREADS) pg_s[b] = pt[b_begin + b];
+        __syncthreads();
+    }
 
     // K chunk c of token j -> chunk c ^ ksw(j); V chunk c -> c ^ vsw(j)   (bank-conflict free)
     auto ksw = [](int j) { return CPR >= 8 ? ((j & 1) << 2) : 0; };
@@ -104,18 +118,27 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
             const int j = c / CPR, part = c % CPR;
             const int tok = t0 + j;
             const bool ok = tok < t_end;
-            const int pg = ok ? pt[tok / a.page] : 0;
+            const int blk = tok >> pshift;
+            const int pg = ok ? (pg_cached ? pg_s[blk - b_begin] : pt[blk]) : 0;
             const bf16_t* kp = a.kv_layer + ((size_t)pg * 2 * a.Hkv + kvh) * head_stride +
-                               (size_t)(ok ? tok % a.page : 0) * HD + part * 8;
+                               (size_t)(ok ? (tok & pmask) : 0) * HD + part * 8;
             const bf16_t* vp = kp + (size_t)a.Hkv * head_stride;
             cp_async16(base + (size_t)j * ROWB + ((part ^ ksw(j)) << 4), kp, ok ? 16 : 0);
             cp_async16(base + (size_t)(ATT_TILE + j) * ROWB + ((part ^ vsw(j)) << 4), vp, ok ? 16 : 0);
         }
     };
-    if (n_tiles > 0) load_tile(0, 0);
-    cp_async_commit();
-    if (n_tiles > 1) load_tile(1, 1);
-    cp_async_commit();
+    // tiles that do not contain the newest position (ctx - 1) can be fetched before the wait
+    const bool early0 = a.prefetch && n_tiles > 0 && (t_begin + ATT_TILE <= ctx - 1);
+    const bool early1 = early0 && n_tiles > 1 && (t_begin + 2 * ATT_TILE <= ctx - 1);
+    if (early0) load_tile(0, 0);
+    if (early0) cp_async_commit();
+    if (early1) load_tile(1, 1);
+    if (early1) cp_async_commit();
+    if (a.prefetch) pdl_wait();
+    trace_mark(13);
+    pdl_launch();
+    if (!early0) { if (n_tiles > 0) load_tile(0, 0); cp_async_commit(); }
+    if (!early1) { if (n_tiles > 1) load_tile(1, 1); cp_async_commit(); }
 
     // Q fragments (hi in rows g, lo in rows g+8), pre-scaled by 1/sqrt(hd); head g of this kv head
     uint32_t qf[KB][8];
@@ -243,7 +266,7 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
             a.part_o[(((size_t)row * a.Hq + hq) * nsp + split) * HD + d] = ov;
         }
     }
-    if (nsp == 1) return;
+    if (nsp == 1) { trace_mark(3 * 4 + 2); return; }
     if (tid < r) {
         const int hq = kvh * r + tid;
         float* ml = a.part_ml + (((size_t)row * a.Hq + hq) * nsp + split) * 2;
@@ -260,24 +283,40 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     if (!last_s) return;
     __threadfence();
     // ---- merge: this CTA arrived last for (row, kvh) -----------------------------------------
+    // warp w computes the normalised weight of every split for heads w, w+4 (lanes = splits) ...
+    float* wgt = &o_w[0][0][0];                       // [r][nsp] (o_w is free again)
+    for (int h = warp; h < r; h += 4) {
+        const int hq = kvh * r + h;
+        const float* ml = a.part_ml + ((size_t)row * a.Hq + hq) * nsp * 2;
+        float mv[2], lv[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const int s2 = lane + 32 * u;
+            mv[u] = (s2 < nsp) ? __ldcg(ml + 2 * s2) : -INFINITY;
+            lv[u] = (s2 < nsp) ? __ldcg(ml + 2 * s2 + 1) : 0.f;
+        }
+        const float mx = warp_max(fmaxf(mv[0], mv[1]));
+        float f[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) f[u] = (lv[u] > 0.f) ? __expf(mv[u] - mx) : 0.f;
+        const float den = warp_sum(f[0] * lv[0] + f[1] * lv[1]);
+#pragma unroll
+        for (int u = 0; u < 2; ++u)
+            if (lane + 32 * u < nsp) wgt[h * nsp + lane + 32 * u] = f[u] / den;
+    }
+    __syncthreads();
+    // ... then every thread combines its output columns (independent loads)
     for (int i = tid; i < r * HD; i += ATT_THREADS) {
         const int h = i / HD, d = i % HD;
         const int hq = kvh * r + h;
-        const float* ml = a.part_ml + ((size_t)row * a.Hq + hq) * nsp * 2;
-        float mx = -INFINITY;
-        for (int s2 = 0; s2 < nsp; ++s2) mx = fmaxf(mx, __ldcg(ml + 2 * s2));
-        float num = 0.f, den = 0.f;
-        for (int s2 = 0; s2 < nsp; ++s2) {
-            const float l2 = __ldcg(ml + 2 * s2 + 1);
-            if (l2 > 0.f) {
-                const float f = __expf(__ldcg(ml + 2 * s2) - mx);
-                num += f * __ldcg(a.part_o + (((size_t)row * a.Hq + hq) * nsp + s2) * HD + d);
-                den += f * l2;
-            }
-        }
-        store_out(a, row, hq * HD + d, num / den);
+        const float* po = a.part_o + ((size_t)row * a.Hq + hq) * nsp * HD + d;
+        float num = 0.f;
+#pragma unroll 4
+        for (int s2 = 0; s2 < nsp; ++s2) num += wgt[h * nsp + s2] * __ldcg(po + (size_t)s2 * HD);
+        store_out(a, row, hq * HD + d, num);
     }
     if (tid == 0) a.counters[row * a.Hkv + kvh] = 0;
+    trace_mark(3 * 4 + 2);
 }
 
 template <int HD>

@@ -72,4 +72,30 @@ __device__ __forceinline__ float warp_max(float v) {
     return v;
 }
 
+// ---- optional in-kernel timeline (build with SAGC_TRACE_BUILD=1: -DSAGC_TRACE -rdc=true) -----
+// thread 0 of block (0,0,0) appends (tag, %globaltimer) records; tag = kernel id * 4 + phase
+// (0 = entered, 1 = upstream dependency satisfied, 2 = block 0 done).  Compiled out by default.
+#ifdef SAGC_TRACE
+extern __device__ unsigned long long* g_trace;
+__device__ __forceinline__ void trace_mark(int tag) {
+    if (g_trace != nullptr && threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        const unsigned long long i = atomicAdd(g_trace, 1ull);
+        if (i < (1ull << 20) - 2) g_trace[1 + i] = ((unsigned long long)tag << 56) | (t & 0x00ffffffffffffffull);
+    }
+}
+__device__ __forceinline__ void trace_mark_thread(int tag, int thread) {
+    if (g_trace != nullptr && (int)threadIdx.x == thread && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        const unsigned long long i = atomicAdd(g_trace, 1ull);
+        if (i < (1ull << 20) - 2) g_trace[1 + i] = ((unsigned long long)tag << 56) | (t & 0x00ffffffffffffffull);
+    }
+}
+#else
+#define trace_mark(tag) ((void)0)
+#define trace_mark_thread(tag, thread) ((void)0)
+#endif
+
 }  // namespace sagc

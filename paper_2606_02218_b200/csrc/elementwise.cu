@@ -7,7 +7,7 @@ namespace sagc {
 // x[row][:] = embed[tok[row]][:] widened to fp32.  One CTA per row, 8 elements per thread-iteration.
 __global__ void __launch_bounds__(128) k_embed(const bf16_t* __restrict__ embed, const int* __restrict__ tok,
                                                const int* m_dev, int m_max, int d, float* __restrict__ x) {
-    pdl_wait();
+    trace_mark(0); pdl_wait(); trace_mark(1);
     pdl_launch();
     const int M = m_dev ? min(*m_dev, m_max) : m_max;
     const int row = blockIdx.x;
@@ -35,7 +35,7 @@ int launch_embed(const bf16_t* embed, const int* tok, const int* m_dev, int m_ma
 // and written to slot pos%page of page page_table[sid][pos/page] -- the ONLY rounding point of
 // the forward pass (reading C1).  grid = (rows, Hq+2*Hkv heads), block = hd/2 threads.
 __global__ void k_rope_append(RopeArgs a) {
-    pdl_wait();
+    trace_mark(8); pdl_wait(); trace_mark(9);
     pdl_launch();
     const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
     const int row = blockIdx.x;
@@ -123,7 +123,7 @@ __global__ void __launch_bounds__(256) k_embed_split(const bf16_t* __restrict__ 
                                                      const bf16_t* __restrict__ norm_w, bf16_t* __restrict__ xs,
                                                      float* __restrict__ ssq, int ssq_ld, int ssq_tiles) {
     __shared__ float red[8];
-    pdl_wait();
+    trace_mark(4); pdl_wait(); trace_mark(5);
     pdl_launch();
     const int M = m_dev ? min(*m_dev, m_max) : m_max;
     const int row = blockIdx.x;

@@ -64,10 +64,12 @@ struct AttnArgs {
     float* out;             // [M][Hq*hd] fp32 (used when out_split is null)
     bf16_t* out_split;      // pre-split rows [2m] = hi, [2m+1] = lo, row stride ld_split (tcgen05 path)
     int ld_split;
+    int prefetch;           // 1 in decode: cached positions older than the newest one predate the upstream kernel
 };
 int launch_attention(const AttnArgs& a, cudaStream_t st);
 
 // Sampler over fp32 logits.  Step a3 / a12.
+static constexpr int SMP_CHUNKS = 32;
 struct SampleArgs {
     const float* logits;    // [M][V]
     int V;
@@ -76,7 +78,8 @@ struct SampleArgs {
     const int* m_dev; int m_max;
     const uint32_t* params; // device [4] = mode, temperature (float bits), Philox key lo, key hi
     int row_div;            // logits row of activation row i is i / row_div (first token: G)
-    int* out_tok;           // [M]
+    float* part_score;      // [M][SMP_CHUNKS] best perturbed score of each vocabulary slice
+    int* part_tok;          // [M][SMP_CHUNKS] and its token id (0x7fffffff if the slice is empty)
 };
 int launch_sample(const SampleArgs& a, cudaStream_t st);
 int launch_philox_debug(uint64_t seed, int sid, int t, int v0, int n, uint32_t* out, cudaStream_t st);
@@ -106,8 +109,8 @@ int launch_pool_reset(const PageState& ps, const RolloutDev& rd, cudaStream_t st
 int launch_prefill_alloc(const PageState& ps, const RolloutDev& rd, cudaStream_t st);
 // End of step t (retire / free / compact) + start of step t+1 (page alloc, pos/ctx/tok).
 // `sampled` holds the sampler's token for each live slot; first_step: slots are sids (t = 1).
-int launch_advance(const PageState& ps, const RolloutDev& rd, const int* sampled, int structure_only,
-                   cudaStream_t st);
+int launch_advance(const PageState& ps, const RolloutDev& rd, const float* part_score, const int* part_tok,
+                   int structure_only, cudaStream_t st);
 // Prefill helpers: row_sid/row_pos/row_ctx/tok for every prompt token, and the copy of a partial
 // last prompt block into the first private page of completions g >= 1.
 int launch_prefill_rows(const int* prompt_tokens, const int* prompt_offsets_dev, int n_prompts, int G,

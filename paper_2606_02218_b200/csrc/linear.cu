@@ -368,18 +368,18 @@ __global__ void __launch_bounds__(LIN_THREADS) k_linear_narrow(LinDev a) {
 // L2-resident), split hi/lo on the fly and fed to HMMA.  SPLITK: the 8 warps of a CTA share one
 // 16-row tile and interleave the 32-wide k blocks (narrow N); otherwise one tile per warp.
 // ---------------------------------------------------------------------------------------
-template <int EPI, bool SPLITK>
-__global__ void __launch_bounds__(LIN_THREADS) k_linear_tail(LinDev a) {
+template <int EPI, bool SPLITK, int NW>
+__global__ void __launch_bounds__(NW * 32) k_linear_tail(LinDev a) {
     constexpr int NS = (EPI == EPI_SWIGLU) ? 2 : 1;
     constexpr int U = 4;                                   // k blocks in flight per warp
-    __shared__ float red[SPLITK ? NS * LIN_WARPS * 4 * 32 : 1];
-    __shared__ float ssq_w[LIN_WARPS][8];
+    __shared__ float red[SPLITK ? NS * NW * 4 * 32 : 1];
+    __shared__ float ssq_w[NW][8];
     __shared__ float rstd_s[8];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane >> 2, q = lane & 3;
-    const int row0 = (SPLITK ? blockIdx.x : blockIdx.x * LIN_WARPS + warp) * 16;
+    const int row0 = (SPLITK ? blockIdx.x : blockIdx.x * NW + warp) * 16;
     const bool active = row0 < a.N;
-    const int kb0 = SPLITK ? warp : 0, kbs = SPLITK ? LIN_WARPS : 1;
+    const int kb0 = SPLITK ? warp : 0, kbs = SPLITK ? NW : 1;
     const int n_kb = a.K >> 5;
     const bf16_t* pa[NS]; const bf16_t* pb[NS];
     if (active) {
@@ -408,7 +408,7 @@ __global__ void __launch_bounds__(LIN_THREADS) k_linear_tail(LinDev a) {
     };
 #pragma unroll
     for (int u = 0; u < U; ++u) load_w(u, kb0 + u * kbs);
-    pdl_wait();
+    trace_mark(16); pdl_wait(); trace_mark(17);
     pdl_launch();
     const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
     if (M <= 0) return;
@@ -479,14 +479,14 @@ __global__ void __launch_bounds__(LIN_THREADS) k_linear_tail(LinDev a) {
 #pragma unroll
         for (int s = 0; s < NS; ++s)
 #pragma unroll
-            for (int e = 0; e < 4; ++e) red[((s * LIN_WARPS + warp) * 4 + e) * 32 + lane] = acc[s][e];
+            for (int e = 0; e < 4; ++e) red[((s * NW + warp) * 4 + e) * 32 + lane] = acc[s][e];
     }
     __syncthreads();
     if (a.norm_w != nullptr && threadIdx.x < 8) {
         float t = 0.f;
         if (SPLITK) {
 #pragma unroll
-            for (int wi = 0; wi < LIN_WARPS; ++wi) t += ssq_w[wi][threadIdx.x];
+            for (int wi = 0; wi < NW; ++wi) t += ssq_w[wi][threadIdx.x];
         }
         rstd_s[threadIdx.x] = t;
     }
@@ -504,7 +504,7 @@ __global__ void __launch_bounds__(LIN_THREADS) k_linear_tail(LinDev a) {
             for (int e = 0; e < 4; ++e) {
                 float t = 0.f;
 #pragma unroll
-                for (int wi = 0; wi < LIN_WARPS; ++wi) t += red[((s * LIN_WARPS + wi) * 4 + e) * 32 + lane];
+                for (int wi = 0; wi < NW; ++wi) t += red[((s * NW + wi) * 4 + e) * 32 + lane];
                 r[s][0][e] = t;
             }
         float rs[8];
@@ -658,14 +658,14 @@ __global__ void __launch_bounds__(LIN_THREADS) k_linear_gemv(LinDev a) {
 // launcher
 // ---------------------------------------------------------------------------------------
 template <typename Kern>
-static cudaError_t launch_cfg(Kern kern, dim3 grid, int smem, bool pdl, cudaStream_t st, LinDev d) {
+static cudaError_t launch_cfg(Kern kern, dim3 grid, int smem, bool pdl, cudaStream_t st, LinDev d, int threads = LIN_THREADS) {
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid;
-    cfg.blockDim = dim3(LIN_THREADS);
+    cfg.blockDim = dim3(threads);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
     cudaLaunchAttribute at[1];
@@ -689,8 +689,13 @@ static cudaError_t launch_epi(const LinearArgs& a, const LinDev& d, cudaStream_t
     }
     const bool wide = tiles >= 148 * LIN_WARPS;
     if (a.m_max <= 8) {
-        if (wide) return launch_cfg(k_linear_tail<EPI, false>, dim3((tiles + LIN_WARPS - 1) / LIN_WARPS), 0, a.pdl, st, d);
-        return launch_cfg(k_linear_tail<EPI, true>, dim3(tiles), 0, a.pdl, st, d);
+        if (wide) return launch_cfg(k_linear_tail<EPI, false, 8>, dim3((tiles + 7) / 8), 0, a.pdl, st, d, 256);
+        // narrow N: one 16-row tile per CTA, the warps interleave the k blocks.  Pick the warp count so
+        // that the grid is ONE wave (small CTAs co-reside) and long K gets more warps (fewer load rounds).
+        const int n_kb = a.K / 32;
+        if (tiles > 148 * 2) return launch_cfg(k_linear_tail<EPI, true, 4>, dim3(tiles), 0, a.pdl, st, d, 128);
+        if (n_kb >= 96 && tiles <= 148) return launch_cfg(k_linear_tail<EPI, true, 16>, dim3(tiles), 0, a.pdl, st, d, 512);
+        return launch_cfg(k_linear_tail<EPI, true, 8>, dim3(tiles), 0, a.pdl, st, d, 256);
     }
     int nt = a.m_max <= 16 ? 2 : (a.m_max <= 32 ? 4 : 8);
     const int my = (a.m_max + nt * 8 - 1) / (nt * 8);

@@ -119,11 +119,11 @@ int launch_prefill_alloc(const PageState& ps, const RolloutDev& rd, cudaStream_t
 }
 
 // End of step t + start of step t+1.  One CTA, thread i = live slot i.
-__global__ void __launch_bounds__(PG_THREADS) k_advance(PageState ps, RolloutDev rd, const int* sampled,
-                                                        int structure_only) {
+__global__ void __launch_bounds__(PG_THREADS) k_advance(PageState ps, RolloutDev rd, const float* part_score,
+                                                        const int* part_tok, int structure_only) {
     __shared__ int warp_s[33];
     __shared__ int grp_live[1024], grp_ret[1024], grp_last[1024];
-    pdl_wait();
+    trace_mark(28); pdl_wait(); trace_mark(29);
     pdl_launch();
     const int i = threadIdx.x;
     const int n_live = *ps.n_live;
@@ -140,7 +140,16 @@ __global__ void __launch_bounds__(PG_THREADS) k_advance(PageState ps, RolloutDev
         sid = ps.live[i];
         grp = sid / rd.G;
         if (rd.forced_tok) tokv = rd.forced_tok[(size_t)sid * rd.max_new + (t - 1)];
-        else if (!structure_only) tokv = sampled[i];
+        else if (!structure_only) {
+            // best of the sampler's per-slice candidates, ascending slices: lowest index wins ties
+            float bs = part_score[i * SMP_CHUNKS];
+            tokv = part_tok[i * SMP_CHUNKS];
+            for (int c = 1; c < SMP_CHUNKS; ++c) {
+                const float s2 = part_score[i * SMP_CHUNKS + c];
+                const int t2 = part_tok[i * SMP_CHUNKS + c];
+                if (s2 > bs || (s2 == bs && t2 < tokv)) { bs = s2; tokv = t2; }
+            }
+        }
         rd.out_tokens[(size_t)sid * rd.max_new + (t - 1)] = tokv;
         rd.out_lengths[sid] = t;
         fin = (rd.forced_len && rd.forced_len[sid] == t) || (rd.stop_token >= 0 && tokv == rd.stop_token) ||
@@ -221,9 +230,9 @@ __global__ void __launch_bounds__(PG_THREADS) k_advance(PageState ps, RolloutDev
         *ps.step = t + 1;
     }
 }
-int launch_advance(const PageState& ps, const RolloutDev& rd, const int* sampled, int structure_only,
-                   cudaStream_t st) {
-    k_advance<<<1, PG_THREADS, 0, st>>>(ps, rd, sampled, structure_only);
+int launch_advance(const PageState& ps, const RolloutDev& rd, const float* part_score, const int* part_tok,
+                   int structure_only, cudaStream_t st) {
+    k_advance<<<1, PG_THREADS, 0, st>>>(ps, rd, part_score, part_tok, structure_only);
     return 1;
 }
 

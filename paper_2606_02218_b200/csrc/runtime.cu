@@ -15,6 +15,23 @@
 
 using namespace sagc;
 
+#ifdef SAGC_TRACE
+namespace sagc { __device__ unsigned long long* g_trace = nullptr; }
+static unsigned long long* g_trace_host = nullptr;
+extern "C" int sagc_debug_trace(unsigned long long* out, long long cap, long long* n) {
+    if (!g_trace_host) { *n = 0; return 0; }
+    cudaDeviceSynchronize();
+    unsigned long long cnt = 0;
+    cudaMemcpy(&cnt, g_trace_host, 8, cudaMemcpyDeviceToHost);
+    if ((long long)cnt > cap) cnt = cap;
+    if (cnt > (1ull << 20) - 2) cnt = (1ull << 20) - 2;
+    cudaMemcpy(out, g_trace_host + 1, cnt * 8, cudaMemcpyDeviceToHost);
+    cudaMemset(g_trace_host, 0, 8);
+    *n = (long long)cnt;
+    return 0;
+}
+#endif
+
 static thread_local char g_err[512] = "";
 static int set_err(int code, const char* fmt, ...) {
     va_list ap;
@@ -62,6 +79,7 @@ struct sagc_model {
     PageState ps;
     // scratch activations
     float *x, *qkv, *att, *act, *logits, *xlast, *part_o, *part_ml;
+    float* part_score;
     int *counters, *sampled, *row_sid, *row_pos, *row_ctx, *row_tok, *last_idx, *prompt_len_d, *offs_d;
     int row_cap;
     // per-call device buffers (grown on demand)
@@ -130,6 +148,13 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return set_err(SAGC_ECUDA, "no CUDA device (there is no CPU fallback)");
 
+#ifdef SAGC_TRACE
+    if (!g_trace_host && env_int("SAGC_TRACE", 0)) {
+        cudaMalloc(&g_trace_host, (1ull << 20) * 8);
+        cudaMemset(g_trace_host, 0, 8);
+        cudaMemcpyToSymbol(sagc::g_trace, &g_trace_host, sizeof(g_trace_host));
+    }
+#endif
     sagc_model* m = new sagc_model();
     m->cfg = c;
     m->own_stream = nullptr; m->own_event = nullptr;
@@ -197,7 +222,7 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     DA(m->part_ml, (size_t)c.max_seqs * c.n_q_heads * m->max_splits * 2);
     DA(m->counters, R * c.n_kv_heads);
     cudaMemset(m->counters, 0, R * c.n_kv_heads * sizeof(int));
-    DA(m->sampled, c.max_seqs); DA(m->last_idx, c.max_seqs); DA(m->prompt_len_d, c.max_seqs);
+    DA(m->sampled, (size_t)c.max_seqs * SMP_CHUNKS); DA(m->part_score, (size_t)c.max_seqs * SMP_CHUNKS); DA(m->last_idx, c.max_seqs); DA(m->prompt_len_d, c.max_seqs);
     DA(m->offs_d, c.max_seqs + 1);
     DA(m->sample_params_d, 4);
     m->last_nseq = 0; m->last_max_blocks = m->max_blocks;
@@ -287,7 +312,7 @@ static int enqueue_layers(sagc_model* m, const RowSet& rs, int n_splits, int kin
         aa.max_blocks = m->max_blocks; aa.row_sid = rs.sid; aa.row_ctx = rs.ctx; aa.m_dev = rs.m_dev; aa.m_max = rs.m_max;
         aa.Hq = c.n_q_heads; aa.Hkv = c.n_kv_heads; aa.hd = c.head_dim; aa.page = c.page_tokens;
         aa.n_splits = n_splits; aa.part_o = m->part_o; aa.part_ml = m->part_ml; aa.counters = m->counters;
-        aa.out = m->att;
+        aa.out = m->att; aa.prefetch = (rs.m_dev != nullptr) ? 1 : 0;
         if (!(skip & 1)) LAUNCH(launch_attention(aa, st));
 
         LinearArgs o = {};
@@ -343,7 +368,7 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cuda
         aa.max_blocks = m->max_blocks; aa.row_sid = rs.sid; aa.row_ctx = rs.ctx; aa.m_dev = rs.m_dev; aa.m_max = rs.m_max;
         aa.Hq = c.n_q_heads; aa.Hkv = c.n_kv_heads; aa.hd = c.head_dim; aa.page = c.page_tokens;
         aa.n_splits = n_splits; aa.part_o = m->part_o; aa.part_ml = m->part_ml; aa.counters = m->counters;
-        aa.out = m->att; aa.out_split = m->att_s; aa.ld_split = qd;
+        aa.out = m->att; aa.prefetch = (rs.m_dev != nullptr) ? 1 : 0; aa.out_split = m->att_s; aa.ld_split = qd;
         if (!(skip & 1)) LAUNCH(launch_attention(aa, st));
 
         TcLinearArgs o = {};
@@ -413,7 +438,8 @@ static int round_bucket(int live) {
 
 static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
     const int ctas = m_bucket * m->cfg.n_kv_heads;
-    int want = (2 * 148 + ctas - 1) / ctas;
+    int want = 222 / ctas;                     // ~1.5 CTAs per SM; no split once the grid fills the chip
+    if (want < 1) want = 1;
     int cap = ctx_bound / 128;
     if (cap < 1) cap = 1;
     if (want > cap) want = cap;
@@ -437,12 +463,12 @@ static int enqueue_decode_step(sagc_model* m, const RolloutDev& rd, int m_bucket
     SampleArgs sa = {};
     sa.logits = m->logits; sa.V = m->cfg.vocab; sa.row_sid = m->ps.live; sa.step_dev = m->ps.step;
     sa.m_dev = m->ps.n_live; sa.m_max = m_bucket; sa.params = m->sample_params_d; sa.row_div = 1;
-    sa.out_tok = m->sampled;
+    sa.part_score = m->part_score; sa.part_tok = m->sampled;
     if (!(m->skip_mask & 2)) n += launch_sample(sa, st);
     if (n_dump > 0)
         n += launch_dump_logits(m->dump_list_d, n_dump, m->ps.step, m->ps.live, m->ps.n_live, 1, m->logits,
                                 m->cfg.vocab, dump_out, st);
-    n += launch_advance(m->ps, rd, m->sampled, 0, st);
+    n += launch_advance(m->ps, rd, m->part_score, m->sampled, 0, st);
     return n;
 }
 
@@ -610,13 +636,13 @@ extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, c
         launches += r;
         SampleArgs sa = {};
         sa.logits = m->logits; sa.V = c.vocab; sa.row_sid = m->ps.live; sa.step_dev = m->ps.step;
-        sa.m_dev = m->ps.n_live; sa.m_max = nseq; sa.params = m->sample_params_d; sa.row_div = G; sa.out_tok = m->sampled;
+        sa.m_dev = m->ps.n_live; sa.m_max = nseq; sa.params = m->sample_params_d; sa.row_div = G; sa.part_score = m->part_score; sa.part_tok = m->sampled;
         launches += launch_sample(sa, st);
         if (prm->n_dump > 0)
             launches += launch_dump_logits(m->dump_list_d, prm->n_dump, m->ps.step, m->ps.live, m->ps.n_live, G,
                                            m->logits, c.vocab, prm->dump_logits, st);
     }
-    launches += launch_advance(m->ps, rd, m->sampled, structure_only ? 1 : 0, st);     // end of step 1
+    launches += launch_advance(m->ps, rd, m->part_score, m->sampled, structure_only ? 1 : 0, st);     // end of step 1
     if (want_t) e_pf = mark();
 
     // ---- decode loop: steps t = 2 .. ---------------------------------------------------
@@ -660,7 +686,7 @@ extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, c
             timing->phase_bytes[ph] += Wb + KVB * (gl * (double)pmax + (double)live * (t - 1)) + KVB * live;
         }
         if (structure_only) {
-            launches += launch_advance(m->ps, rd, m->sampled, 1, st);
+            launches += launch_advance(m->ps, rd, m->part_score, m->sampled, 1, st);
         } else {
             const int mb = round_bucket(live);
             const int ns = pick_splits(m, mb, pmax + t - 1);

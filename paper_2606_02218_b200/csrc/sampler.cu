@@ -40,17 +40,19 @@ int launch_philox_debug(uint64_t seed, int sid, int t, int v0, int n, uint32_t* 
     return 1;
 }
 
-static constexpr int SMP_THREADS = 1024;
+static constexpr int SMP_THREADS = 256;
 
 __device__ __forceinline__ void better(float& bs, int& bi, float s, int i) {
     if (s > bs || (s == bs && i < bi)) { bs = s; bi = i; }
 }
 
-// one CTA per row
+// grid = (rows, SMP_CHUNKS): each CTA scans one contiguous slice of the vocabulary and writes its
+// best (score, index); the step-advance kernel takes the best of the SMP_CHUNKS partials in
+// ascending chunk order (lowest index wins exact ties).
 __global__ void __launch_bounds__(SMP_THREADS) k_sample(SampleArgs a) {
-    __shared__ float ws[32];
-    __shared__ int wi[32];
-    pdl_wait();
+    __shared__ float ws[8];
+    __shared__ int wi[8];
+    trace_mark(24); pdl_wait(); trace_mark(25);
     pdl_launch();
     const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
     const int row = blockIdx.x;
@@ -64,7 +66,9 @@ __global__ void __launch_bounds__(SMP_THREADS) k_sample(SampleArgs a) {
     float bs = -INFINITY;
     int bi = 0x7fffffff;
     const int nblk = (a.V + 3) >> 2;
-    for (int b = threadIdx.x; b < nblk; b += SMP_THREADS) {
+    const int per = (nblk + SMP_CHUNKS - 1) / SMP_CHUNKS;
+    const int b_lo = blockIdx.y * per, b_hi = min(nblk, b_lo + per);
+    for (int b = b_lo + threadIdx.x; b < b_hi; b += SMP_THREADS) {
         const int v = b << 2;
         float s[4];
         if (v + 3 < a.V) {
@@ -92,21 +96,16 @@ __global__ void __launch_bounds__(SMP_THREADS) k_sample(SampleArgs a) {
     }
     if ((threadIdx.x & 31) == 0) { ws[threadIdx.x >> 5] = bs; wi[threadIdx.x >> 5] = bi; }
     __syncthreads();
-    if (threadIdx.x < 32) {
-        bs = ws[threadIdx.x]; bi = wi[threadIdx.x];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            float s2 = __shfl_xor_sync(0xffffffffu, bs, o);
-            int i2 = __shfl_xor_sync(0xffffffffu, bi, o);
-            better(bs, bi, s2, i2);
-        }
-        if (threadIdx.x == 0) a.out_tok[row] = bi;
+    if (threadIdx.x == 0) {
+        for (int w2 = 1; w2 < SMP_THREADS / 32; ++w2) better(bs, bi, ws[w2], wi[w2]);
+        a.part_score[row * SMP_CHUNKS + blockIdx.y] = bs;
+        a.part_tok[row * SMP_CHUNKS + blockIdx.y] = bi;
     }
 }
 
 int launch_sample(const SampleArgs& a, cudaStream_t st) {
     if (a.m_max <= 0) return 0;
-    k_sample<<<a.m_max, SMP_THREADS, 0, st>>>(a);
+    k_sample<<<dim3(a.m_max, SMP_CHUNKS), SMP_THREADS, 0, st>>>(a);
     return 1;
 }
 

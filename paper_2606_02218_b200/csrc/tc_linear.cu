@@ -14,6 +14,8 @@
 #include <cooperative_groups.h>
 #include <cuda.h>
 
+#include <cstdlib>
+
 #include "common.cuh"
 #include "kernels.cuh"
 
@@ -112,6 +114,7 @@ struct TcDev {
     float* ssq_out;                 // EPI_RESID: [N/128][ssq_ld] partial sums of squares of the new x
     const float* ssq_in; int ssq_in_tiles;   // fused RMSNorm of the INPUT: rstd[m] from these partials
     int ssq_ld; float eps; int k_norm;
+    int stages;                     // smem ring depth chosen by the launcher
 };
 
 template <int NB, int NA>
@@ -119,11 +122,13 @@ struct TcCfg {
     static constexpr int A_BYTES = 128 * 128;
     static constexpr int B_BYTES = NB * 128;
     static constexpr int STAGE = NA * A_BYTES + B_BYTES;
-    static constexpr int STAGES = STAGE <= 32 * 1024 ? 6 : (STAGE <= 48 * 1024 ? 4 : 3);
+    // ~100 KB of stages per CTA so that two CTAs share an SM (one's epilogue overlaps the other's loads)
+    static constexpr int STAGES = (100 * 1024 / STAGE) < 2 ? 2 : ((100 * 1024 / STAGE) > 6 ? 6 : (100 * 1024 / STAGE));
     static constexpr int MB = NB / 2;
     static constexpr int TMEM_COLS = NA * NB <= 32 ? 32 : (NA * NB <= 64 ? 64 : (NA * NB <= 128 ? 128 : (NA * NB <= 256 ? 256 : 512)));
     static constexpr int TAIL = 1024;                                  // barriers, tmem slot, rstd, ssq scratch
-    static constexpr int SMEM = STAGES * STAGE + TAIL + 5 * MB * 4 + 1024;   // + alignment slack
+    static constexpr int MAXSTAGES = (196 * 1024 / STAGE) > 8 ? 8 : (196 * 1024 / STAGE);
+    static constexpr int smem_bytes(int stages) { return stages * STAGE + TAIL + 5 * MB * 4 + 1024; }
 };
 
 __device__ __forceinline__ float silu_tc(float z) { return z / (1.f + __expf(-z)); }
@@ -135,7 +140,8 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             TcDev a) {
     constexpr int NA = (EPI == EPI_SWIGLU) ? 2 : 1;
     using C = TcCfg<NB, NA>;
-    constexpr int S = C::STAGES, MB = C::MB;
+    constexpr int MB = C::MB;
+    const int S = a.stages;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem + S * C::STAGE);
@@ -178,6 +184,9 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
+    float res_first[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) res_first[j] = 0.f;
     if (warp == 0) {
         // ===== TMA producer =====
         if (lane == 0) {
@@ -192,7 +201,7 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
                 tma_load_2d(st, mapA, &full[i], (kb0 + i) * TC_BK, arow);
                 if (EPI == EPI_SWIGLU) tma_load_2d(st + C::A_BYTES, &tmA2, &full[i], (kb0 + i) * TC_BK, arow);
             }
-            pdl_wait();
+            trace_mark(5 * 4); pdl_wait(); trace_mark(5 * 4 + 1);
             for (int i = 0; i < pre; ++i)
                 tma_load_2d(smem + i * C::STAGE + NA * C::A_BYTES, &tmB, &full[i], (kb0 + i) * TC_BK, 2 * m0);
             for (int i = pre; i < nk; ++i) {
@@ -205,6 +214,7 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
                 tma_load_2d(st + NA * C::A_BYTES, &tmB, &full[s], (kb0 + i) * TC_BK, 2 * m0);
             }
         }
+        trace_mark(8 * 4 + 0);
         pdl_launch();
     } else if (warp == 1) {
         // ===== MMA issuer =====
@@ -243,10 +253,19 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
                 rstd_s[m] = rsqrtf(t / (float)a.k_norm + a.eps);
             }
         }
+        if (EPI == EPI_RESID) {
+            const int Mv = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const int mn = min(rank + j * KS, MB - 1);
+                res_first[j] = a.R[(size_t)max(min(m0 + mn, Mv - 1), 0) * a.ldy + row0 + row];
+            }
+        }
         if (nk > 0) {
             mbar_wait(accum, 0);
             tc_fence_after();
         }
+        trace_mark_thread(8 * 4 + 1, 64);
 #pragma unroll
         for (int na = 0; na < NA; ++na) {
 #pragma unroll
@@ -263,56 +282,98 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             }
         }
         tc_fence_before();
+        trace_mark_thread(8 * 4 + 2, 64);
     }
     cluster.sync();            // every partial tile of the cluster is in shared memory
+    trace_mark_thread(8 * 4 + 3, 64);
     if (warp >= 2) {
         const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
         const int lg = warp & 3;
         const int row = lg * 32 + lane;
         const int n = row0 + row;
-        const float* peer[8];
-#pragma unroll
-        for (int p = 0; p < 8; ++p) peer[p] = (p < KS) ? cluster.map_shared_rank(red, p) : red;
         float nw = 1.f;
         if (EPI == EPI_RESID && a.norm_next != nullptr) nw = bf16_to_f32(a.norm_next[n]);
-        for (int m = rank; m < MB; m += KS) {
-            const int mg = m0 + m;
-            if (mg >= M) break;
-            float acc[NA];
+        constexpr int MBATCH = 8;                 // columns in flight: DSMEM / L2 latency is paid once per batch
+        // residual values of the NEXT batch are fetched while the current one is finished (the first
+        // batch was requested before the accumulator wait, see res_first)
+        float res_nxt[MBATCH];
 #pragma unroll
-            for (int na = 0; na < NA; ++na) {
-                float t = 0.f;
+        for (int j = 0; j < MBATCH; ++j) res_nxt[j] = res_first[j];
+        for (int mb = rank; mb < MB; mb += KS * MBATCH) {
+            float acc[MBATCH][NA];
+            float res[MBATCH];
+            // all loads of a batch are unconditional (indices clamped) so that they issue back to back:
+            // one shared-memory / DSMEM / L2 round trip per rank and batch instead of one per column
+            int mc[MBATCH];
 #pragma unroll
-                for (int p = 0; p < 8; ++p)
-                    if (p < KS) t += peer[p][((size_t)na * MB + m) * 128 + row];
-                acc[na] = t;
+            for (int j = 0; j < MBATCH; ++j) {
+                mc[j] = min(mb + j * KS, MB - 1);
+#pragma unroll
+                for (int na = 0; na < NA; ++na) acc[j][na] = 0.f;
+                res[j] = res_nxt[j];
+                if (EPI == EPI_RESID) {
+                    const int mn = min(mb + KS * MBATCH + j * KS, MB - 1);
+                    res_nxt[j] = a.R[(size_t)max(min(m0 + mn, M - 1), 0) * a.ldy + n];
+                }
             }
-            const float sc = (a.ssq_in != nullptr) ? rstd_s[m] : 1.f;
-            if (EPI == EPI_STORE) {
-                a.Y[(size_t)mg * a.ldy + n] = acc[0] * sc;
-            } else if (EPI == EPI_RESID) {
-                const size_t o = (size_t)mg * a.ldy + n;
-                const float xn = a.R[o] + acc[0] * sc;
-                a.Y[o] = xn;
-                if (a.xs_out != nullptr) {
-                    const float xw = xn * nw;
-                    const uint32_t hi = f32_to_bf16_bits(xw);
-                    const uint32_t lo = f32_to_bf16_bits(xw - __uint_as_float(hi << 16));
-                    a.xs_out[(size_t)(2 * mg) * a.ld_xs + n] = (bf16_t)hi;
-                    a.xs_out[(size_t)(2 * mg + 1) * a.ld_xs + n] = (bf16_t)lo;
-                }
-                if (a.ssq_out != nullptr) {
-                    const float q2 = warp_sum(xn * xn);
-                    if (lane == 0) ssq_s[lg * MB + m] = q2;
-                }
+            if (KS == 1) {
+#pragma unroll
+                for (int j = 0; j < MBATCH; ++j)
+#pragma unroll
+                    for (int na = 0; na < NA; ++na) acc[j][na] = red[((size_t)na * MB + mc[j]) * 128 + row];
             } else {
-                const float v = silu_tc(acc[0] * sc) * (acc[NA - 1] * sc);
-                const uint32_t hi = f32_to_bf16_bits(v);
-                const uint32_t lo = f32_to_bf16_bits(v - __uint_as_float(hi << 16));
-                a.xs_out[(size_t)(2 * mg) * a.ld_xs + n] = (bf16_t)hi;
-                a.xs_out[(size_t)(2 * mg + 1) * a.ld_xs + n] = (bf16_t)lo;
+                for (int p = 0; p < KS; ++p) {
+                    const float* pr = cluster.map_shared_rank(red, p);
+                    float v[MBATCH][NA];
+#pragma unroll
+                    for (int j = 0; j < MBATCH; ++j)
+#pragma unroll
+                        for (int na = 0; na < NA; ++na) v[j][na] = pr[((size_t)na * MB + mc[j]) * 128 + row];
+#pragma unroll
+                    for (int j = 0; j < MBATCH; ++j)
+#pragma unroll
+                        for (int na = 0; na < NA; ++na) acc[j][na] += v[j][na];
+                }
+            }
+            // branch-free per-column math (the 8 columns interleave: the epilogue warps run one per
+            // scheduler, so instruction-level parallelism is the only latency hiding there is)
+            float outv[MBATCH], q2[MBATCH];
+            uint32_t ohi[MBATCH], olo[MBATCH];
+#pragma unroll
+            for (int j = 0; j < MBATCH; ++j) {
+                const float sc = (a.ssq_in != nullptr) ? rstd_s[mc[j]] : 1.f;
+                float v;
+                if (EPI == EPI_STORE) v = acc[j][0] * sc;
+                else if (EPI == EPI_RESID) v = res[j] + acc[j][0] * sc;
+                else v = silu_tc(acc[j][0] * sc) * (acc[j][NA - 1] * sc);
+                outv[j] = v;
+                const float xw = (EPI == EPI_RESID) ? v * nw : v;
+                ohi[j] = f32_to_bf16_bits(xw);
+                olo[j] = f32_to_bf16_bits(xw - __uint_as_float(ohi[j] << 16));
+                q2[j] = v * v;
+            }
+            if (EPI == EPI_RESID && a.ssq_out != nullptr) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                    for (int j = 0; j < MBATCH; ++j) q2[j] += __shfl_xor_sync(0xffffffffu, q2[j], o);
+            }
+#pragma unroll
+            for (int j = 0; j < MBATCH; ++j) {
+                const int m = mb + j * KS;
+                const int mg = m0 + m;
+                const bool ok = m < MB && mg < M;
+                if (ok) {
+                    if (EPI != EPI_SWIGLU) a.Y[(size_t)mg * a.ldy + n] = outv[j];
+                    if (EPI != EPI_STORE && a.xs_out != nullptr) {
+                        a.xs_out[(size_t)(2 * mg) * a.ld_xs + n] = (bf16_t)ohi[j];
+                        a.xs_out[(size_t)(2 * mg + 1) * a.ld_xs + n] = (bf16_t)olo[j];
+                    }
+                    if (EPI == EPI_RESID && a.ssq_out != nullptr && lane == 0) ssq_s[lg * MB + m] = q2[j];
+                }
             }
         }
+        trace_mark_thread(9 * 4 + 1, 64);
         if (EPI == EPI_RESID && a.ssq_out != nullptr) {
             asm volatile("bar.sync 1, 128;\n" ::: "memory");
             const int et = (warp - 2) * 32 + lane;
@@ -323,8 +384,10 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             }
         }
     }
+    trace_mark_thread(9 * 4 + 2, 64);
     tc_fence_before();
     cluster.sync();            // peers may still be reading this CTA's shared memory
+    trace_mark(5 * 4 + 2);
     if (warp == 2) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "n"(C::TMEM_COLS));
@@ -382,10 +445,16 @@ int tc_make_map(TcMap* out, const void* base, long long rows, int K, int box_row
 template <int NB, int EPI>
 static cudaError_t launch_tc_inst(const TcLinearArgs& t, const TcDev& d, dim3 grid, int KS, cudaStream_t st) {
     constexpr int NA = (EPI == EPI_SWIGLU) ? 2 : 1;
-    const int smem = TcCfg<NB, NA>::SMEM;
+    using C = TcCfg<NB, NA>;
+    // grids that fit the chip in one wave get the deepest ring; multi-wave grids (LM head, prefill) keep
+    // ~100 KB so two CTAs share an SM and one's epilogue overlaps the other's loads
+    const bool one_wave = (long long)grid.x * grid.y * grid.z <= 148;
+    const int stages = one_wave ? C::MAXSTAGES : C::STAGES;
+    const int smem = C::smem_bytes(stages);
+    TcDev d2 = d; d2.stages = stages;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_linear_tc<NB, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(k_linear_tc<NB, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::smem_bytes(C::MAXSTAGES));
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
@@ -407,7 +476,7 @@ static cudaError_t launch_tc_inst(const TcLinearArgs& t, const TcDev& d, dim3 gr
     const CUtensorMap* b = reinterpret_cast<const CUtensorMap*>(t.b);
     const int seg0 = t.a[1] ? t.seg_rows[0] : t.N + 128;
     const int seg1 = t.a[2] ? t.seg_rows[0] + t.seg_rows[1] : t.N + 128;
-    return cudaLaunchKernelEx(&cfg, k_linear_tc<NB, EPI>, *a0, *a1, *a2, *b, seg0, seg1, d);
+    return cudaLaunchKernelEx(&cfg, k_linear_tc<NB, EPI>, *a0, *a1, *a2, *b, seg0, seg1, d2);
 }
 
 int tc_nb_index(int m_max) { return m_max <= 16 ? 0 : (m_max <= 32 ? 1 : (m_max <= 64 ? 2 : 3)); }
@@ -421,7 +490,15 @@ int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
     const int nbi = tc_nb_index(t.m_max);
     const int NB = 32 << nbi, MB = NB / 2;
     const int tiles = t.N / 128, mtiles = (t.m_max + MB - 1) / MB;
-    int KS = 148 / (tiles * mtiles);
+    // K-split policy (measured with the in-kernel timeline): a CTA streams its weight slab through a deep
+    // TMA ring at well over 150 GB/s, while every extra cluster rank adds DSMEM round trips to the
+    // epilogue -- so K is split only down to ~120 KB slabs per CTA (swept on cfg2) and never beyond two CTAs per SM.
+    const int NAh = (t.epi == EPI_SWIGLU) ? 2 : 1;
+    const double slab = (double)NAh * 128.0 * t.K * 2.0;
+    static const double slab_max = [] { const char* e = getenv("SAGC_TC_SLAB_KB"); return (e ? atof(e) : 120.0) * 1e3; }();
+    int KS = (int)((slab + slab_max - 1) / slab_max);
+    const int room = (2 * 148) / (tiles * mtiles);
+    if (KS > room) KS = room;
     if (KS < 1) KS = 1;
     if (KS > 8) KS = 8;
     if (KS > d.n_kb) KS = d.n_kb;
