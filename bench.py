@@ -128,6 +128,16 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def allreduce_max(values, device, world):
+    """Max over ranks of a few scalars (the timed region of the slowest replica is the job's time)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), device=device, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
 def kernel_roofline(B, torch, mc, peak):
     """Time the largest single launch of a decode step alone (LM head, M = 64): CUDA events on the
     launching stream, weights (272 MB) larger than L2 so every iteration streams from HBM."""
@@ -240,10 +250,7 @@ def main():
         peak, peak_src = measured_peaks()
         kr = kernel_roofline(B, torch, mc, peak) if rank == 0 else None
 
-    tms = torch.tensor([ms, e2e_s * 1e3], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-    ms, e2e_ms = float(tms[0]), float(tms[1])
+    ms, e2e_ms = allreduce_max([ms, e2e_s * 1e3], "cuda", world)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
