@@ -93,7 +93,16 @@ __device__ __forceinline__ void trace_mark_thread(int tag, int thread) {
         if (i < (1ull << 20) - 2) g_trace[1 + i] = ((unsigned long long)tag << 56) | (t & 0x00ffffffffffffffull);
     }
 }
+__device__ __forceinline__ void trace_mark_allblocks(int tag) {
+    if (g_trace != nullptr && threadIdx.x == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        const unsigned long long i = atomicAdd(g_trace, 1ull);
+        if (i < (1ull << 20) - 2) g_trace[1 + i] = ((unsigned long long)tag << 56) | (t & 0x00ffffffffffffffull);
+    }
+}
 #else
+#define trace_mark_allblocks(tag) ((void)0)
 #define trace_mark(tag) ((void)0)
 #define trace_mark_thread(tag, thread) ((void)0)
 #endif

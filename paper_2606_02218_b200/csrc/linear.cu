@@ -12,8 +12,14 @@
 //   mode B (narrow N, e.g. O / down projections): one 16-row tile per CTA, the 8 warps
 //          interleave the 32-wide k blocks and reduce through shared memory (fixed order).
 // A separate fp32-activation GEMV kernel (LIN_GEMV) serves the straggler tail.
+#include <cooperative_groups.h>
+
+#include <cstdlib>
+
 #include "common.cuh"
 #include "kernels.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace sagc {
 
@@ -379,8 +385,14 @@ __global__ void __launch_bounds__(NW * 32) k_linear_tail(LinDev a) {
     const int g = lane >> 2, q = lane & 3;
     const int row0 = (SPLITK ? blockIdx.x : blockIdx.x * NW + warp) * 16;
     const bool active = row0 < a.N;
-    const int kb0 = SPLITK ? warp : 0, kbs = SPLITK ? NW : 1;
-    const int n_kb = a.K >> 5;
+    // narrow N with long K: a cluster of KC CTAs splits K (rank = blockIdx.y), reduced through DSMEM
+    cg::cluster_group cluster = cg::this_cluster();
+    const int KC = SPLITK ? (int)cluster.num_blocks() : 1;
+    const int crank = SPLITK ? (int)cluster.block_rank() : 0;
+    const int kb_all = a.K >> 5;
+    const int kb_per = (kb_all + KC - 1) / KC;
+    const int kb0 = crank * kb_per + (SPLITK ? warp : 0), kbs = SPLITK ? NW : 1;
+    const int n_kb = min(kb_all, (crank + 1) * kb_per);
     const bf16_t* pa[NS]; const bf16_t* pb[NS];
     if (active) {
         if (EPI == EPI_SWIGLU) {
@@ -469,6 +481,7 @@ __global__ void __launch_bounds__(NW * 32) k_linear_tail(LinDev a) {
             }
         }
     }
+    trace_mark_allblocks(4 * 4 + 2);
     // row sums of squares: lanes (g, q = 0..3) hold disjoint k slices of batch row g
     if (a.norm_w != nullptr) {
         ssq += __shfl_xor_sync(0xffffffffu, ssq, 1);
@@ -496,25 +509,43 @@ __global__ void __launch_bounds__(NW * 32) k_linear_tail(LinDev a) {
     }
     __syncthreads();
     if (SPLITK) {
-        if (warp != 0) return;
+        __shared__ float cred[NS * 4 * 32 + 8];
         float r[NS][1][4];
+        if (warp == 0) {
 #pragma unroll
-        for (int s = 0; s < NS; ++s)
+            for (int s = 0; s < NS; ++s)
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                float t = 0.f;
+                for (int e = 0; e < 4; ++e) {
+                    float t = 0.f;
 #pragma unroll
-                for (int wi = 0; wi < NW; ++wi) t += red[((s * NW + wi) * 4 + e) * 32 + lane];
-                r[s][0][e] = t;
+                    for (int wi = 0; wi < NW; ++wi) t += red[((s * NW + wi) * 4 + e) * 32 + lane];
+                    r[s][0][e] = t;
+                }
+            if (KC > 1 && crank != 0) {
+#pragma unroll
+                for (int s = 0; s < NS; ++s)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) cred[(s * 4 + e) * 32 + lane] = r[s][0][e];
+                if (lane < 8) cred[NS * 4 * 32 + lane] = rstd_s[lane];
             }
-        float rs[8];
-        if (a.norm_w != nullptr) {
-            // in-warp: lanes 0..7 convert the sums, everyone reads through smem (same warp)
-            if (lane < 8) rstd_s[lane] = rsqrtf(rstd_s[lane] / (float)a.K + a.eps);
-            __syncwarp();
         }
-        (void)rs;
-        if (active) epilogue<1, EPI>(a, r[0], r[NS - 1], row0, 0, M, rstd_s, lane);
+        if (KC > 1) cluster.sync();
+        if (warp == 0 && crank == 0) {
+            for (int p = 1; p < KC; ++p) {                         // rank order: deterministic
+                const float* pc = cluster.map_shared_rank(cred, p);
+#pragma unroll
+                for (int s = 0; s < NS; ++s)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) r[s][0][e] += pc[(s * 4 + e) * 32 + lane];
+                if (lane < 8) rstd_s[lane] += pc[NS * 4 * 32 + lane];
+            }
+            if (a.norm_w != nullptr) {
+                if (lane < 8) rstd_s[lane] = rsqrtf(rstd_s[lane] / (float)a.K + a.eps);
+                __syncwarp();
+            }
+            if (active) epilogue<1, EPI>(a, r[0], r[NS - 1], row0, 0, M, rstd_s, lane);
+        }
+        if (KC > 1) cluster.sync();                                // keep cred alive until rank 0 has read it
     } else {
         float* mine = ssq_w[warp];
         if (a.norm_w != nullptr) {
@@ -658,7 +689,8 @@ __global__ void __launch_bounds__(LIN_THREADS) k_linear_gemv(LinDev a) {
 // launcher
 // ---------------------------------------------------------------------------------------
 template <typename Kern>
-static cudaError_t launch_cfg(Kern kern, dim3 grid, int smem, bool pdl, cudaStream_t st, LinDev d, int threads = LIN_THREADS) {
+static cudaError_t launch_cfg(Kern kern, dim3 grid, int smem, bool pdl, cudaStream_t st, LinDev d, int threads = LIN_THREADS,
+                              int cluster_y = 1) {
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
@@ -668,11 +700,20 @@ static cudaError_t launch_cfg(Kern kern, dim3 grid, int smem, bool pdl, cudaStre
     cfg.blockDim = dim3(threads);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchAttribute at[2];
+    int na = 0;
+    if (pdl) {
+        at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    if (cluster_y > 1) {
+        at[na].id = cudaLaunchAttributeClusterDimension;
+        at[na].val.clusterDim.x = 1; at[na].val.clusterDim.y = cluster_y; at[na].val.clusterDim.z = 1;
+        ++na;
+    }
     cfg.attrs = at;
-    cfg.numAttrs = pdl ? 1 : 0;
+    cfg.numAttrs = na;
     return cudaLaunchKernelEx(&cfg, kern, d);
 }
 
@@ -694,6 +735,9 @@ static cudaError_t launch_epi(const LinearArgs& a, const LinDev& d, cudaStream_t
         // that the grid is ONE wave (small CTAs co-reside) and long K gets more warps (fewer load rounds).
         const int n_kb = a.K / 32;
         if (tiles > 148 * 2) return launch_cfg(k_linear_tail<EPI, true, 4>, dim3(tiles), 0, a.pdl, st, d, 128);
+        if (n_kb >= 96 && tiles <= 74 && getenv("SAGC_TAIL_CLUSTER")) {   // optional: K split over a 2-CTA cluster (DSMEM reduce)
+            return launch_cfg(k_linear_tail<EPI, true, 16>, dim3(tiles, 2), 0, a.pdl, st, d, 512, 2);
+        }
         if (n_kb >= 96 && tiles <= 148) return launch_cfg(k_linear_tail<EPI, true, 16>, dim3(tiles), 0, a.pdl, st, d, 512);
         return launch_cfg(k_linear_tail<EPI, true, 8>, dim3(tiles), 0, a.pdl, st, d, 256);
     }
