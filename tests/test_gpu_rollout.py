@@ -248,7 +248,7 @@ def _sampled_parity(B, cfg, n_prompts, P, G, max_new, fl, path, n_dump_seq=3):
     assert np.array_equal(lens, np.minimum(fl, max_new))
     st, _ = opg.run_structure_only(n_pages, w.model.page_tokens, [P] * n_prompts, G, fl, max_new)
     _check_structure(B, m, st, out, lens)
-    dec = odec.RefDecoder(w.model, weights)
+    dec = odec.RefDecoder(w.model, weights, cache_f32=w.model.n_params() < 1e9)
     lg = out.dump_logits.cpu().numpy()
     worst, n_bad, n_dis, n_all = 0.0, 0, 0, 0
     for sid in sids:
@@ -274,3 +274,17 @@ def test_config2_truncated(B, path):
     """0.5B shape: 2 prompts x 256 x G=8 (16 live -> tcgen05 path, then the tail path below 9 live)."""
     fl = np.array([3, 14, 14, 2, 14, 9, 5, 14, 14, 1, 14, 7, 14, 14, 4, 14], dtype=np.int32)
     _sampled_parity(B, 2, 2, 256, 8, 14, fl, path)
+
+
+def test_config3_truncated(B):
+    """1.5B shape (head_dim 128, r = 6, DAPO config): 1 prompt x 96 tokens (ragged vs the 64-token page) x G=16."""
+    fl = np.array([10, 3, 10, 10, 1, 10, 7, 10, 10, 10, 5, 10, 10, 2, 10, 10], dtype=np.int32)
+    _sampled_parity(B, 3, 1, 96, 16, 10, fl, 0, n_dump_seq=2)
+
+
+@pytest.mark.parametrize("cfg,G", [(4, 32)])
+def test_config4_truncated(B, cfg, G):
+    """7B shape (configs 4 and 5 share it): 1 prompt x 128 tokens x G=32 -> 32 live rows on the tcgen05 path,
+    then the tail path; logits of two sampled sequences against the fp32 oracle."""
+    fl = np.array([6, 4, 6, 3, 6, 2, 6, 1, 6, 4, 6, 3] + [1, 2, 3, 4] * 5, dtype=np.int32)   # 6 live in steps 5-6
+    _sampled_parity(B, cfg, 1, 128, G, 6, fl, 0, n_dump_seq=2)
