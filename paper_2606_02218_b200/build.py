@@ -19,6 +19,8 @@ SOURCES = ["linear.cu", "tc_linear.cu", "attention.cu", "elementwise.cu", "sampl
 HEADERS = ["common.cuh", "kernels.cuh", os.path.join("..", "..", "include", "sagc.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
+if os.environ.get("SAGC_PDL_EARLY"):
+    NVCC_FLAGS += ["-DSAGC_PDL_EARLY"]
 if os.environ.get("SAGC_TRACE_BUILD"):       # in-kernel timeline (debug builds only)
     NVCC_FLAGS += ["-DSAGC_TRACE", "-rdc=true"]
 

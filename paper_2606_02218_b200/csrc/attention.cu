@@ -328,7 +328,7 @@ static int launch_att(const AttnArgs& a, cudaStream_t st) {
         attr_set = true;
     }
     dim3 grid(a.m_max, a.Hkv, a.n_splits);
-    k_attention<HD><<<grid, ATT_THREADS, AttSmem<HD>::BYTES, st>>>(a);
+    launch_pdl(k_attention<HD>, grid, dim3(ATT_THREADS), AttSmem<HD>::BYTES, st, g_pdl_all, a);
     return 1;
 }
 

@@ -57,7 +57,17 @@ __device__ __forceinline__ void prefetch_l2(const void* p) {
 // ---- programmatic dependent launch (griddepcontrol) ---------------------------------
 // pdl_wait(): block until the upstream grid's memory is visible (no-op without the PDL attr).
 // pdl_launch(): allow the downstream grid to start its prologue.
+// SAGC_PDL_EARLY: release the downstream grid BEFORE waiting on the upstream one, so that the launch
+// chain runs ahead of execution and several kernels' weight prefetches are in flight at once
+// (a kernel's wait still implies, transitively, that every earlier kernel of the stream is complete).
+#ifdef SAGC_PDL_EARLY
+__device__ __forceinline__ void pdl_wait() {
+    asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+    asm volatile("griddepcontrol.wait;\n" ::: "memory");
+}
+#else
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;\n" ::: "memory"); }
+#endif
 __device__ __forceinline__ void pdl_launch() { asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory"); }
 
 // ---- warp reductions -------------------------------------------------------------
@@ -106,5 +116,23 @@ __device__ __forceinline__ void trace_mark_allblocks(int tag) {
 #define trace_mark(tag) ((void)0)
 #define trace_mark_thread(tag, thread) ((void)0)
 #endif
+
+// Launch with the programmatic-stream-serialization attribute (PDL): the kernel may start while its
+// predecessor is still running and must call pdl_wait() before touching anything the predecessor wrote.
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl,
+                                     Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
 
 }  // namespace sagc

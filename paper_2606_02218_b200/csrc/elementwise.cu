@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(128) k_embed(const bf16_t* __restrict__ embed,
 int launch_embed(const bf16_t* embed, const int* tok, const int* m_dev, int m_max, int d, float* x,
                  cudaStream_t st) {
     if (m_max <= 0) return 0;
-    k_embed<<<m_max, 128, 0, st>>>(embed, tok, m_dev, m_max, d, x);
+    launch_pdl(k_embed, dim3(m_max), dim3(128), 0, st, g_pdl_all, embed, tok, m_dev, m_max, d, x);
     return 1;
 }
 
@@ -72,7 +72,7 @@ __global__ void k_rope_append(RopeArgs a) {
 int launch_rope_append(const RopeArgs& a, cudaStream_t st) {
     if (a.m_max <= 0) return 0;
     dim3 grid(a.m_max, a.Hq + 2 * a.Hkv);
-    k_rope_append<<<grid, a.hd / 2, 0, st>>>(a);
+    launch_pdl(k_rope_append, grid, dim3(a.hd / 2), 0, st, g_pdl_all, a);
     return 1;
 }
 
@@ -152,7 +152,7 @@ __global__ void __launch_bounds__(256) k_embed_split(const bf16_t* __restrict__ 
 int launch_embed_split(const bf16_t* embed, const int* tok, const int* m_dev, int m_max, int d, float* x,
                        const bf16_t* norm_w, bf16_t* xs, float* ssq, int ssq_ld, int ssq_tiles, cudaStream_t st) {
     if (m_max <= 0) return 0;
-    k_embed_split<<<m_max, 256, 0, st>>>(embed, tok, m_dev, m_max, d, x, norm_w, xs, ssq, ssq_ld, ssq_tiles);
+    launch_pdl(k_embed_split, dim3(m_max), dim3(256), 0, st, g_pdl_all, embed, tok, m_dev, m_max, d, x, norm_w, xs, ssq, ssq_ld, ssq_tiles);
     return 1;
 }
 

@@ -8,6 +8,8 @@ namespace sagc {
 
 typedef uint16_t bf16_t;   // raw bf16 bit pattern
 
+extern bool g_pdl_all;     // launch the small kernels (embed, rope, attention, sampler, advance) with the PDL attribute too
+
 enum { EPI_STORE = 0, EPI_RESID = 1, EPI_SWIGLU = 2 };
 enum { LIN_MMA = 0, LIN_GEMV = 1, LIN_TC = 2 };
 

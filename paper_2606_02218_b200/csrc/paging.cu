@@ -232,7 +232,7 @@ __global__ void __launch_bounds__(PG_THREADS) k_advance(PageState ps, RolloutDev
 }
 int launch_advance(const PageState& ps, const RolloutDev& rd, const float* part_score, const int* part_tok,
                    int structure_only, cudaStream_t st) {
-    k_advance<<<1, PG_THREADS, 0, st>>>(ps, rd, part_score, part_tok, structure_only);
+    launch_pdl(k_advance, dim3(1), dim3(PG_THREADS), 0, st, g_pdl_all, ps, rd, part_score, part_tok, structure_only);
     return 1;
 }
 

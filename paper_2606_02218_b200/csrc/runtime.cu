@@ -15,6 +15,8 @@
 
 using namespace sagc;
 
+namespace sagc { bool g_pdl_all = false; }
+
 #ifdef SAGC_TRACE
 namespace sagc { __device__ unsigned long long* g_trace = nullptr; }
 static unsigned long long* g_trace_host = nullptr;
@@ -175,6 +177,7 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     m->page_elems = (size_t)2 * c.n_kv_heads * c.page_tokens * c.head_dim;
     m->layer_stride = m->page_elems * (size_t)c.n_pages;
     m->use_pdl = env_int("SAGC_PDL", 1) != 0;
+    sagc::g_pdl_all = m->use_pdl && env_int("SAGC_PDL_ALL", 1) != 0;
     m->gemv_max = env_int("SAGC_GEMV_MAX", 0);
     m->skip_mask = env_int("SAGC_SKIP", 0);
     m->tok_buf = m->len_buf = m->forced_len_d = m->dump_list_d = m->prompt_tok_d = nullptr;

@@ -105,7 +105,7 @@ __global__ void __launch_bounds__(SMP_THREADS) k_sample(SampleArgs a) {
 
 int launch_sample(const SampleArgs& a, cudaStream_t st) {
     if (a.m_max <= 0) return 0;
-    k_sample<<<dim3(a.m_max, SMP_CHUNKS), SMP_THREADS, 0, st>>>(a);
+    launch_pdl(k_sample, dim3(a.m_max, SMP_CHUNKS), dim3(SMP_THREADS), 0, st, g_pdl_all, a);
     return 1;
 }
 
