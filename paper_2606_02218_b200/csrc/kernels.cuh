@@ -131,6 +131,7 @@ int launch_dump_logits(const int* dump_sid_t, int n_dump, const int* step_dev, c
 struct alignas(64) TcMap { unsigned char opaque[128]; };     // mirrors CUtensorMap
 int tc_make_map(TcMap* out, const void* base, long long rows, int K, int box_rows);
 int tc_nb_index(int m_max);                                  // 0..3 -> UMMA N = 32, 64, 128, 256
+static constexpr size_t TC_SCRATCH_FLOATS = (size_t)296 * 2 * 128 * 128;   // 296 CTAs x NA 2 x 128 cols x 128 rows
 struct TcLinearArgs {
     const TcMap* a[3];          // weight maps (box 64 x 128): {w} | {q, k, v} | {gate, up}
     int seg_rows[3];
@@ -141,6 +142,7 @@ struct TcLinearArgs {
     float* Y; int ldy; const float* R;
     bf16_t* xs_out; int ld_xs; const bf16_t* norm_next; float* ssq_out;
     const float* ssq_in; int ssq_in_tiles; int ssq_ld; float eps; int k_norm;
+    float* scratch;             // >= TC_SCRATCH_FLOATS floats for the split-K partial tiles (null: no K split)
     bool pdl;
 };
 int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st);

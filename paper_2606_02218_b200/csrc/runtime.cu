@@ -99,6 +99,7 @@ struct sagc_model {
     bool tc_ok;
     bf16_t *xs, *att_s, *act_s;
     float* ssq;
+    float* tc_scratch;
     int ssq_ld, d_tiles;
     std::vector<TcMap> wmaps;                  // per layer: q k v o g u d ; last = lm_head
     TcMap amaps[3][4];                         // {xs, att_s, act_s} x UMMA N {32, 64, 128, 256}
@@ -239,6 +240,7 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
             m->ssq_ld = (int)Rp; m->d_tiles = c.d_model / 128;
             DA(m->xs, 2 * Rp * c.d_model); DA(m->att_s, 2 * Rp * qd); DA(m->act_s, 2 * Rp * c.d_ff);
             DA(m->ssq, (size_t)m->d_tiles * Rp);
+            DA(m->tc_scratch, TC_SCRATCH_FLOATS);
             cudaMemset(m->xs, 0, 2 * Rp * c.d_model * 2); cudaMemset(m->att_s, 0, 2 * Rp * qd * 2);
             cudaMemset(m->act_s, 0, 2 * Rp * c.d_ff * 2); cudaMemset(m->ssq, 0, (size_t)m->d_tiles * Rp * 4);
             m->wmaps.resize((size_t)L * 7 + 1);
@@ -356,7 +358,7 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cuda
         t.a[0] = &w7[0]; t.a[1] = &w7[1]; t.a[2] = &w7[2]; t.seg_rows[0] = qd; t.seg_rows[1] = kvd; t.seg_rows[2] = kvd;
         t.b = &m->amaps[0][nbi]; t.K = c.d_model; t.N = m->Nqkv; t.m_dev = rs.m_dev; t.m_max = rs.m_max; t.epi = EPI_STORE;
         t.Y = m->qkv; t.ldy = m->Nqkv; t.ssq_in = m->ssq; t.ssq_in_tiles = m->d_tiles; t.ssq_ld = m->ssq_ld;
-        t.eps = c.rms_eps; t.k_norm = c.d_model; t.pdl = m->use_pdl;
+        t.eps = c.rms_eps; t.k_norm = c.d_model; t.pdl = m->use_pdl; t.scratch = m->tc_scratch;
         if (!(skip & 4)) LAUNCH(launch_linear_tc(t, st));
 
         RopeArgs ra = {};
@@ -378,21 +380,21 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cuda
         o.a[0] = &w7[3]; o.seg_rows[0] = c.d_model; o.b = &m->amaps[1][nbi]; o.K = qd; o.N = c.d_model;
         o.m_dev = rs.m_dev; o.m_max = rs.m_max; o.epi = EPI_RESID; o.Y = m->x; o.R = m->x; o.ldy = c.d_model;
         o.xs_out = m->xs; o.ld_xs = c.d_model; o.norm_next = m->norm2[l]; o.ssq_out = m->ssq; o.ssq_ld = m->ssq_ld;
-        o.eps = c.rms_eps; o.pdl = m->use_pdl;
+        o.eps = c.rms_eps; o.pdl = m->use_pdl; o.scratch = m->tc_scratch;
         if (!(skip & 4)) LAUNCH(launch_linear_tc(o, st));
 
         TcLinearArgs gu = {};
         gu.a[0] = &w7[4]; gu.a[1] = &w7[5]; gu.seg_rows[0] = c.d_ff; gu.seg_rows[1] = c.d_ff;
         gu.b = &m->amaps[0][nbi]; gu.K = c.d_model; gu.N = c.d_ff; gu.m_dev = rs.m_dev; gu.m_max = rs.m_max;
         gu.epi = EPI_SWIGLU; gu.xs_out = m->act_s; gu.ld_xs = c.d_ff; gu.ssq_in = m->ssq; gu.ssq_in_tiles = m->d_tiles;
-        gu.ssq_ld = m->ssq_ld; gu.eps = c.rms_eps; gu.k_norm = c.d_model; gu.pdl = m->use_pdl;
+        gu.ssq_ld = m->ssq_ld; gu.eps = c.rms_eps; gu.k_norm = c.d_model; gu.pdl = m->use_pdl; gu.scratch = m->tc_scratch;
         if (!(skip & 4)) LAUNCH(launch_linear_tc(gu, st));
 
         TcLinearArgs dn = {};
         dn.a[0] = &w7[6]; dn.seg_rows[0] = c.d_model; dn.b = &m->amaps[2][nbi]; dn.K = c.d_ff; dn.N = c.d_model;
         dn.m_dev = rs.m_dev; dn.m_max = rs.m_max; dn.epi = EPI_RESID; dn.Y = m->x; dn.R = m->x; dn.ldy = c.d_model;
         dn.xs_out = m->xs; dn.ld_xs = c.d_model; dn.norm_next = (l + 1 < c.n_layers) ? m->norm1[l + 1] : m->final_norm;
-        dn.ssq_out = m->ssq; dn.ssq_ld = m->ssq_ld; dn.eps = c.rms_eps; dn.pdl = m->use_pdl;
+        dn.ssq_out = m->ssq; dn.ssq_ld = m->ssq_ld; dn.eps = c.rms_eps; dn.pdl = m->use_pdl; dn.scratch = m->tc_scratch;
         if (!(skip & 4)) LAUNCH(launch_linear_tc(dn, st));
     }
     return n;
@@ -409,7 +411,7 @@ static int enqueue_lm_head(sagc_model* m, const float* xsrc, const int* m_dev, i
         t.a[0] = &m->wmaps[(size_t)c.n_layers * 7]; t.seg_rows[0] = c.vocab; t.b = &m->amaps[0][tc_nb_index(m_max)];
         t.K = c.d_model; t.N = c.vocab; t.m_dev = m_dev; t.m_max = m_max; t.epi = EPI_STORE; t.Y = m->logits; t.ldy = c.vocab;
         t.ssq_in = m->ssq; t.ssq_in_tiles = m->d_tiles; t.ssq_ld = m->ssq_ld; t.eps = c.rms_eps; t.k_norm = c.d_model;
-        t.pdl = m->use_pdl;
+        t.pdl = m->use_pdl; t.scratch = m->tc_scratch;
         return launch_linear_tc(t, st);
     }
     if (kind == LIN_TC) kind = LIN_MMA;          // gathered fp32 rows (first token): register HMMA path
@@ -889,10 +891,12 @@ extern "C" int sagc_debug_linear(const void* W, const float* x, float* y, int32_
         }
         TcLinearArgs t = {};
         t.a[0] = &ma; t.seg_rows[0] = N; t.b = &mb; t.K = K; t.N = N; t.m_dev = nullptr; t.m_max = M; t.epi = EPI_STORE;
-        t.Y = y; t.ldy = N; t.pdl = false;
+        float* scr = nullptr;
+        CU(cudaMalloc(&scr, TC_SCRATCH_FLOATS * sizeof(float)));
+        t.Y = y; t.ldy = N; t.pdl = false; t.scratch = scr;
         int r = launch_linear_tc(t, st);
         cudaError_t e = cudaStreamSynchronize(st);
-        cudaFree(xs);
+        cudaFree(xs); cudaFree(scr);
         if (r < 0 || e != cudaSuccess) return set_err(SAGC_ECUDA, "tcgen05 linear: %s", cudaGetErrorString(e != cudaSuccess ? e : cudaGetLastError()));
         return SAGC_OK;
     }

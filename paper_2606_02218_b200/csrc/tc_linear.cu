@@ -115,6 +115,7 @@ struct TcDev {
     const float* ssq_in; int ssq_in_tiles;   // fused RMSNorm of the INPUT: rstd[m] from these partials
     int ssq_ld; float eps; int k_norm;
     int stages;                     // smem ring depth chosen by the launcher
+    float* scratch;                 // split-K partial tiles [cta][NA][MB][128] (L2-resident), KS > 1 only
 };
 
 template <int NB, int NA>
@@ -132,6 +133,96 @@ struct TcCfg {
 };
 
 __device__ __forceinline__ float silu_tc(float z) { return z / (1.f + __expf(-z)); }
+
+// Final epilogue of one CTA: rank r of a KS-way split finishes batch columns r, r+KS, ...  KS is a
+// compile-time constant so that EVERY load of a batch (all ranks' partial tiles from L2, or the local
+// tile from shared memory, plus the residual) is issued before the first use: one memory round trip per
+// batch of 64 / (NA*KS) columns, partials summed in rank order (deterministic).
+template <int NB, int EPI, int KS>
+__device__ __forceinline__ void tc_epilogue(const TcDev& a, const float* red, const float* rstd_s, float* ssq_s, int warp,
+                                            int lane, int row0, int m0, int tile, int rank, int cta_id) {
+    constexpr int NA = (EPI == EPI_SWIGLU) ? 2 : 1;
+    constexpr int MB = NB / 2;
+    constexpr int MBATCH = (KS == 1) ? 16 / NA : 64 / (NA * KS);
+    const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
+    const int lg = warp & 3;
+    const int row = lg * 32 + lane;
+    const int n = row0 + row;
+    float nw = 1.f;
+    if (EPI == EPI_RESID && a.norm_next != nullptr) nw = bf16_to_f32(a.norm_next[n]);
+    const float* base = (KS == 1) ? red : a.scratch + (size_t)(cta_id - rank) * (NA * MB * 128);
+    for (int mb = rank; mb < MB; mb += KS * MBATCH) {
+        if (m0 + mb >= M) break;
+        int mc[MBATCH];
+        float v[KS][MBATCH][NA], res[MBATCH];
+#pragma unroll
+        for (int j = 0; j < MBATCH; ++j) {
+            mc[j] = min(mb + j * KS, MB - 1);
+            res[j] = (EPI == EPI_RESID) ? a.R[(size_t)min(m0 + mc[j], M - 1) * a.ldy + n] : 0.f;
+        }
+#pragma unroll
+        for (int p = 0; p < KS; ++p)
+#pragma unroll
+            for (int j = 0; j < MBATCH; ++j)
+#pragma unroll
+                for (int na = 0; na < NA; ++na) {
+                    const float* src = base + (size_t)p * (NA * MB * 128) + ((size_t)na * MB + mc[j]) * 128 + row;
+                    v[p][j][na] = (KS == 1) ? *src : __ldcg(src);
+                }
+        float outv[MBATCH], q2[MBATCH];
+        uint32_t ohi[MBATCH], olo[MBATCH];
+#pragma unroll
+        for (int j = 0; j < MBATCH; ++j) {
+            float acc[NA];
+#pragma unroll
+            for (int na = 0; na < NA; ++na) {
+                float t = v[0][j][na];
+#pragma unroll
+                for (int p = 1; p < KS; ++p) t += v[p][j][na];
+                acc[na] = t;
+            }
+            const float sc = (a.ssq_in != nullptr) ? rstd_s[mc[j]] : 1.f;
+            float o;
+            if (EPI == EPI_STORE) o = acc[0] * sc;
+            else if (EPI == EPI_RESID) o = res[j] + acc[0] * sc;
+            else o = silu_tc(acc[0] * sc) * (acc[NA - 1] * sc);
+            outv[j] = o;
+            const float xw = (EPI == EPI_RESID) ? o * nw : o;
+            ohi[j] = f32_to_bf16_bits(xw);
+            olo[j] = f32_to_bf16_bits(xw - __uint_as_float(ohi[j] << 16));
+            q2[j] = o * o;
+        }
+        if (EPI == EPI_RESID && a.ssq_out != nullptr) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                for (int j = 0; j < MBATCH; ++j) q2[j] += __shfl_xor_sync(0xffffffffu, q2[j], o);
+        }
+#pragma unroll
+        for (int j = 0; j < MBATCH; ++j) {
+            const int m = mb + j * KS;
+            const int mg = m0 + m;
+            if (m < MB && mg < M) {
+                if (EPI != EPI_SWIGLU) a.Y[(size_t)mg * a.ldy + n] = outv[j];
+                if (EPI != EPI_STORE && a.xs_out != nullptr) {
+                    a.xs_out[(size_t)(2 * mg) * a.ld_xs + n] = (bf16_t)ohi[j];
+                    a.xs_out[(size_t)(2 * mg + 1) * a.ld_xs + n] = (bf16_t)olo[j];
+                }
+                if (EPI == EPI_RESID && a.ssq_out != nullptr && lane == 0) ssq_s[lg * MB + m] = q2[j];
+            }
+        }
+    }
+    trace_mark_thread(9 * 4 + 1, 64);
+    if (EPI == EPI_RESID && a.ssq_out != nullptr) {
+        asm volatile("bar.sync 1, 128;\n" ::: "memory");
+        const int et = (warp - 2) * 32 + lane;
+        for (int m = et; m < MB; m += 128) {
+            if ((m % KS) == rank && m0 + m < M)
+                a.ssq_out[(size_t)tile * a.ssq_ld + m0 + m] =
+                    ssq_s[0 * MB + m] + ssq_s[1 * MB + m] + ssq_s[2 * MB + m] + ssq_s[3 * MB + m];
+        }
+    }
+}
 
 template <int NB, int EPI>
 __global__ void __launch_bounds__(TC_THREADS, 1)
@@ -158,6 +249,7 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tile = blockIdx.x, row0 = tile * 128;
     const int m0 = blockIdx.z * MB;
+    const int cta_id = ((int)blockIdx.z * (int)gridDim.x + (int)blockIdx.x) * KS + rank;
     const int kb0 = rank * a.kb_per_cta;
     const int nk = max(0, min(a.n_kb, kb0 + a.kb_per_cta) - kb0);
 
@@ -184,9 +276,6 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    float res_first[8];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) res_first[j] = 0.f;
     if (warp == 0) {
         // ===== TMA producer =====
         if (lane == 0) {
@@ -253,14 +342,6 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
                 rstd_s[m] = rsqrtf(t / (float)a.k_norm + a.eps);
             }
         }
-        if (EPI == EPI_RESID) {
-            const int Mv = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const int mn = min(rank + j * KS, MB - 1);
-                res_first[j] = a.R[(size_t)max(min(m0 + mn, Mv - 1), 0) * a.ldy + row0 + row];
-            }
-        }
         if (nk > 0) {
             mbar_wait(accum, 0);
             tc_fence_after();
@@ -277,8 +358,14 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 #pragma unroll
                     for (int j = 0; j < 32; ++j) v[j] = 0.f;
                 }
+                if (KS == 1) {
 #pragma unroll
-                for (int j = 0; j < 16; ++j) red[((size_t)na * MB + c * 16 + j) * 128 + row] = v[2 * j] + v[2 * j + 1];
+                    for (int j = 0; j < 16; ++j) red[((size_t)na * MB + c * 16 + j) * 128 + row] = v[2 * j] + v[2 * j + 1];
+                } else {      // split-K partials go through L2: far more bandwidth than DSMEM's ~20 B/clk per SM
+                    float* mine = a.scratch + (size_t)cta_id * (NA * MB * 128);
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) __stcg(mine + ((size_t)na * MB + c * 16 + j) * 128 + row, v[2 * j] + v[2 * j + 1]);
+                }
             }
         }
         tc_fence_before();
@@ -287,101 +374,11 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     cluster.sync();            // every partial tile of the cluster is in shared memory
     trace_mark_thread(8 * 4 + 3, 64);
     if (warp >= 2) {
-        const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
-        const int lg = warp & 3;
-        const int row = lg * 32 + lane;
-        const int n = row0 + row;
-        float nw = 1.f;
-        if (EPI == EPI_RESID && a.norm_next != nullptr) nw = bf16_to_f32(a.norm_next[n]);
-        constexpr int MBATCH = 8;                 // columns in flight: DSMEM / L2 latency is paid once per batch
-        // residual values of the NEXT batch are fetched while the current one is finished (the first
-        // batch was requested before the accumulator wait, see res_first)
-        float res_nxt[MBATCH];
-#pragma unroll
-        for (int j = 0; j < MBATCH; ++j) res_nxt[j] = res_first[j];
-        for (int mb = rank; mb < MB; mb += KS * MBATCH) {
-            float acc[MBATCH][NA];
-            float res[MBATCH];
-            // all loads of a batch are unconditional (indices clamped) so that they issue back to back:
-            // one shared-memory / DSMEM / L2 round trip per rank and batch instead of one per column
-            int mc[MBATCH];
-#pragma unroll
-            for (int j = 0; j < MBATCH; ++j) {
-                mc[j] = min(mb + j * KS, MB - 1);
-#pragma unroll
-                for (int na = 0; na < NA; ++na) acc[j][na] = 0.f;
-                res[j] = res_nxt[j];
-                if (EPI == EPI_RESID) {
-                    const int mn = min(mb + KS * MBATCH + j * KS, MB - 1);
-                    res_nxt[j] = a.R[(size_t)max(min(m0 + mn, M - 1), 0) * a.ldy + n];
-                }
-            }
-            if (KS == 1) {
-#pragma unroll
-                for (int j = 0; j < MBATCH; ++j)
-#pragma unroll
-                    for (int na = 0; na < NA; ++na) acc[j][na] = red[((size_t)na * MB + mc[j]) * 128 + row];
-            } else {
-                for (int p = 0; p < KS; ++p) {
-                    const float* pr = cluster.map_shared_rank(red, p);
-                    float v[MBATCH][NA];
-#pragma unroll
-                    for (int j = 0; j < MBATCH; ++j)
-#pragma unroll
-                        for (int na = 0; na < NA; ++na) v[j][na] = pr[((size_t)na * MB + mc[j]) * 128 + row];
-#pragma unroll
-                    for (int j = 0; j < MBATCH; ++j)
-#pragma unroll
-                        for (int na = 0; na < NA; ++na) acc[j][na] += v[j][na];
-                }
-            }
-            // branch-free per-column math (the 8 columns interleave: the epilogue warps run one per
-            // scheduler, so instruction-level parallelism is the only latency hiding there is)
-            float outv[MBATCH], q2[MBATCH];
-            uint32_t ohi[MBATCH], olo[MBATCH];
-#pragma unroll
-            for (int j = 0; j < MBATCH; ++j) {
-                const float sc = (a.ssq_in != nullptr) ? rstd_s[mc[j]] : 1.f;
-                float v;
-                if (EPI == EPI_STORE) v = acc[j][0] * sc;
-                else if (EPI == EPI_RESID) v = res[j] + acc[j][0] * sc;
-                else v = silu_tc(acc[j][0] * sc) * (acc[j][NA - 1] * sc);
-                outv[j] = v;
-                const float xw = (EPI == EPI_RESID) ? v * nw : v;
-                ohi[j] = f32_to_bf16_bits(xw);
-                olo[j] = f32_to_bf16_bits(xw - __uint_as_float(ohi[j] << 16));
-                q2[j] = v * v;
-            }
-            if (EPI == EPI_RESID && a.ssq_out != nullptr) {
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1)
-#pragma unroll
-                    for (int j = 0; j < MBATCH; ++j) q2[j] += __shfl_xor_sync(0xffffffffu, q2[j], o);
-            }
-#pragma unroll
-            for (int j = 0; j < MBATCH; ++j) {
-                const int m = mb + j * KS;
-                const int mg = m0 + m;
-                const bool ok = m < MB && mg < M;
-                if (ok) {
-                    if (EPI != EPI_SWIGLU) a.Y[(size_t)mg * a.ldy + n] = outv[j];
-                    if (EPI != EPI_STORE && a.xs_out != nullptr) {
-                        a.xs_out[(size_t)(2 * mg) * a.ld_xs + n] = (bf16_t)ohi[j];
-                        a.xs_out[(size_t)(2 * mg + 1) * a.ld_xs + n] = (bf16_t)olo[j];
-                    }
-                    if (EPI == EPI_RESID && a.ssq_out != nullptr && lane == 0) ssq_s[lg * MB + m] = q2[j];
-                }
-            }
-        }
-        trace_mark_thread(9 * 4 + 1, 64);
-        if (EPI == EPI_RESID && a.ssq_out != nullptr) {
-            asm volatile("bar.sync 1, 128;\n" ::: "memory");
-            const int et = (warp - 2) * 32 + lane;
-            for (int m = et; m < MB; m += 128) {
-                if ((m % KS) == rank && m0 + m < M)
-                    a.ssq_out[(size_t)tile * a.ssq_ld + m0 + m] =
-                        ssq_s[0 * MB + m] + ssq_s[1 * MB + m] + ssq_s[2 * MB + m] + ssq_s[3 * MB + m];
-            }
+        switch (KS) {
+            case 1: tc_epilogue<NB, EPI, 1>(a, red, rstd_s, ssq_s, warp, lane, row0, m0, tile, rank, cta_id); break;
+            case 2: tc_epilogue<NB, EPI, 2>(a, red, rstd_s, ssq_s, warp, lane, row0, m0, tile, rank, cta_id); break;
+            case 4: tc_epilogue<NB, EPI, 4>(a, red, rstd_s, ssq_s, warp, lane, row0, m0, tile, rank, cta_id); break;
+            default: tc_epilogue<NB, EPI, 8>(a, red, rstd_s, ssq_s, warp, lane, row0, m0, tile, rank, cta_id); break;
         }
     }
     trace_mark_thread(9 * 4 + 2, 64);
@@ -486,24 +483,25 @@ int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
     TcDev d;
     d.K = t.K; d.N = t.N; d.n_kb = t.K / TC_BK; d.m_dev = t.m_dev; d.m_max = t.m_max; d.Y = t.Y; d.ldy = t.ldy; d.R = t.R;
     d.xs_out = t.xs_out; d.ld_xs = t.ld_xs; d.norm_next = t.norm_next; d.ssq_out = t.ssq_out; d.ssq_in = t.ssq_in;
-    d.ssq_in_tiles = t.ssq_in_tiles; d.ssq_ld = t.ssq_ld; d.eps = t.eps; d.k_norm = t.k_norm;
+    d.ssq_in_tiles = t.ssq_in_tiles; d.ssq_ld = t.ssq_ld; d.eps = t.eps; d.k_norm = t.k_norm; d.scratch = t.scratch;
     const int nbi = tc_nb_index(t.m_max);
     const int NB = 32 << nbi, MB = NB / 2;
     const int tiles = t.N / 128, mtiles = (t.m_max + MB - 1) / MB;
     // K-split policy (measured with the in-kernel timeline): a CTA streams its weight slab through a deep
     // TMA ring at well over 150 GB/s, while every extra cluster rank adds DSMEM round trips to the
-    // epilogue -- so K is split only down to ~120 KB slabs per CTA (swept on cfg2) and never beyond two CTAs per SM.
+    // epilogue -- so K is split down to ~30 KB slabs per CTA (swept on cfg2), in powers of two up to 8, and never beyond two CTAs per SM.
     const int NAh = (t.epi == EPI_SWIGLU) ? 2 : 1;
     const double slab = (double)NAh * 128.0 * t.K * 2.0;
-    static const double slab_max = [] { const char* e = getenv("SAGC_TC_SLAB_KB"); return (e ? atof(e) : 120.0) * 1e3; }();
+    static const double slab_max = [] { const char* e = getenv("SAGC_TC_SLAB_KB"); return (e ? atof(e) : 30.0) * 1e3; }();
     int KS = (int)((slab + slab_max - 1) / slab_max);
     const int room = (2 * 148) / (tiles * mtiles);
     if (KS > room) KS = room;
     if (KS < 1) KS = 1;
     if (KS > 8) KS = 8;
     if (KS > d.n_kb) KS = d.n_kb;
-    d.kb_per_cta = (d.n_kb + KS - 1) / KS;
-    KS = (d.n_kb + d.kb_per_cta - 1) / d.kb_per_cta;
+    if (t.scratch == nullptr) KS = 1;
+    { int p2 = 1; while (p2 * 2 <= KS) p2 *= 2; KS = p2; }      // the epilogue is specialised for 1, 2, 4, 8
+    d.kb_per_cta = (d.n_kb + KS - 1) / KS;             // trailing ranks may get fewer (or zero) k blocks
     dim3 grid(tiles, KS, mtiles);
     cudaError_t e;
 #define TC_CASE(NBV)                                                                         \
