@@ -157,7 +157,7 @@ def kernel_roofline(B, torch, mc, peak):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / n
     nbytes = N * K * 2 + M * K * 4 + M * N * 4
-    return {"kernel": "k_linear_wide<8,STORE> (LM head, M=64)", "bytes": nbytes, "ms": ms,
+    return {"kernel": "k_linear_tc<128,STORE> (LM head, 64 live rows; + k_split_rows)", "bytes": nbytes, "ms": ms,
             "achieved_gbs": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak}
 
 

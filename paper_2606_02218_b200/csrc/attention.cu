@@ -165,9 +165,11 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
         for (int e = 0; e < 4; ++e) o[n][e] = 0.f;
     float m_run = -INFINITY, l_run = 0.f;       // head g (replicated over the quad)
 
+    trace_mark(10 * 4 + 0);
     for (int tile = 0; tile < n_tiles; ++tile) {
         cp_async_wait<1>();
-        __syncthreads();                         // tile landed; the stage of tile-1 is free
+        __syncthreads();
+        if (tile == 0) trace_mark(10 * 4 + 1);                         // tile landed; the stage of tile-1 is free
         if (tile + 2 < n_tiles) load_tile(tile + 2, (tile + 2) % ATT_STAGES);
         cp_async_commit();
         const unsigned char* kbase = kv_s + (size_t)(tile % ATT_STAGES) * AttSmem<HD>::STAGE;
@@ -233,6 +235,7 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
         }
     }
     cp_async_wait<0>();
+    trace_mark(10 * 4 + 2);
     // ---- merge the four warps (fixed order) ---------------------------------------------------
     // lane (g, q) holds head g: o[n][0..1] + o[n][2..3] are columns n*8 + 2q, +1
     if (g < r) {
@@ -273,6 +276,7 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
         ml[0] = m_s[tid];
         ml[1] = l_s[tid];
     }
+    trace_mark(10 * 4 + 3);
     __threadfence();
     __syncthreads();
     if (tid == 0) {

@@ -443,7 +443,8 @@ static int round_bucket(int live) {
 
 static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
     const int ctas = m_bucket * m->cfg.n_kv_heads;
-    int want = 222 / ctas;                     // ~1.5 CTAs per SM; no split once the grid fills the chip
+    static const int target = env_int("SAGC_ATT_CTAS", 222);
+    int want = target / ctas;                  // ~1.5 CTAs per SM; no split once the grid fills the chip
     if (want < 1) want = 1;
     int cap = ctx_bound / 128;
     if (cap < 1) cap = 1;
@@ -879,25 +880,29 @@ extern "C" int sagc_debug_linear(const void* W, const float* x, float* y, int32_
     if (path == SAGC_PATH_GEMM && N % 128 == 0 && K % 64 == 0) {
         // tcgen05 path: pre-split the activations, build the two tensor maps, one launch
         const int nbi = tc_nb_index(M), NB = 32 << nbi;
-        bf16_t* xs = nullptr;
+        static bf16_t* xs = nullptr;            // debug entry: grow-only buffers, kept for the process lifetime
+        static size_t xs_cap = 0;
         const size_t rows = 2 * (size_t)(((M + NB / 2 - 1) / (NB / 2)) * (NB / 2));
-        CU(cudaMalloc(&xs, rows * K * sizeof(bf16_t)));
-        CU(cudaMemsetAsync(xs, 0, rows * K * sizeof(bf16_t), st));
+        if (rows * K > xs_cap) {
+            CU(cudaDeviceSynchronize());
+            if (xs) cudaFree(xs);
+            xs_cap = rows * K;
+            CU(cudaMalloc(&xs, xs_cap * sizeof(bf16_t)));
+            CU(cudaMemset(xs, 0, xs_cap * sizeof(bf16_t)));
+        }
         launch_split_rows(x, K, nullptr, M, xs, st);
         TcMap ma, mb;
         if (tc_make_map(&ma, W, N, K, 128) != 0 || tc_make_map(&mb, xs, (long long)rows, K, NB) != 0) {
-            cudaFree(xs);
             return set_err(SAGC_ECUDA, "cuTensorMapEncodeTiled failed");
         }
         TcLinearArgs t = {};
         t.a[0] = &ma; t.seg_rows[0] = N; t.b = &mb; t.K = K; t.N = N; t.m_dev = nullptr; t.m_max = M; t.epi = EPI_STORE;
-        float* scr = nullptr;
-        CU(cudaMalloc(&scr, TC_SCRATCH_FLOATS * sizeof(float)));
+        static float* scr = nullptr;            // debug entry: allocated once per process
+        if (!scr) CU(cudaMalloc(&scr, TC_SCRATCH_FLOATS * sizeof(float)));
         t.Y = y; t.ldy = N; t.pdl = false; t.scratch = scr;
         int r = launch_linear_tc(t, st);
-        cudaError_t e = cudaStreamSynchronize(st);
-        cudaFree(xs); cudaFree(scr);
-        if (r < 0 || e != cudaSuccess) return set_err(SAGC_ECUDA, "tcgen05 linear: %s", cudaGetErrorString(e != cudaSuccess ? e : cudaGetLastError()));
+        if (r < 0) return set_err(SAGC_ECUDA, "tcgen05 linear: %s", cudaGetErrorString(cudaGetLastError()));
+        CU(cudaGetLastError());
         return SAGC_OK;
     }
     // rows beyond 64 are processed by the kernels' own m-chunk grid dimension

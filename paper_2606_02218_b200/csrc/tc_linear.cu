@@ -371,8 +371,14 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         tc_fence_before();
         trace_mark_thread(8 * 4 + 2, 64);
     }
-    cluster.sync();            // every partial tile of the cluster is in shared memory
+    // every rank's partial tile is now in the L2 scratch (KS > 1) or in this CTA's shared memory (KS == 1);
+    // all tcgen05.ld of this CTA have completed, so the TMEM columns can go back right away
+    if (KS > 1) cluster.sync(); else __syncthreads();
     trace_mark_thread(8 * 4 + 3, 64);
+    if (warp == 2) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "n"(C::TMEM_COLS));
+    }
     if (warp >= 2) {
         switch (KS) {
             case 1: tc_epilogue<NB, EPI, 1>(a, red, rstd_s, ssq_s, warp, lane, row0, m0, tile, rank, cta_id); break;
@@ -381,14 +387,9 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             default: tc_epilogue<NB, EPI, 8>(a, red, rstd_s, ssq_s, warp, lane, row0, m0, tile, rank, cta_id); break;
         }
     }
+    // no second cluster barrier: peers read this CTA's partials from the L2 scratch, never from its
+    // shared memory, so the CTA may retire as soon as its own columns are written
     trace_mark_thread(9 * 4 + 2, 64);
-    tc_fence_before();
-    cluster.sync();            // peers may still be reading this CTA's shared memory
-    trace_mark(5 * 4 + 2);
-    if (warp == 2) {
-        tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "n"(C::TMEM_COLS));
-    }
 }
 
 // ---- x fp32 [M][K] -> pre-split rows (test / debug entry and embedding path) ---------------
