@@ -405,6 +405,14 @@ __global__ void __launch_bounds__(NW * 32) k_linear_tail(LinDev a) {
             pb[0] = seg_row(a, row0 + g + 8) + 8 * q;
         }
     }
+    // Ask L2 for this CTA's whole weight slab right away (one bulk prefetch per row): the DRAM reads then
+    // overlap the upstream kernel and the later register loads of the k loop hit L2.
+    if (SPLITK && active && warp == 0 && lane < 16 * NS) {
+        const int s = lane >> 4, rr = lane & 15;
+        const bf16_t* rowp = (EPI == EPI_SWIGLU) ? ((s == 0 ? a.W0 : a.W1) + (size_t)(row0 + rr) * a.K)
+                                                 : seg_row(a, row0 + rr);
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(rowp), "r"(a.K * 2) : "memory");
+    }
     uint4 w[NS][U][2];
     auto load_w = [&](int u, int kb) {
 #pragma unroll
