@@ -94,6 +94,7 @@ struct sagc_model {
     int last_nseq, last_max_blocks;
     bool use_pdl;
     int gemv_max;
+    int tc_min;                                // smallest live-row bucket routed to the tcgen05 path
     int skip_mask;                             // SAGC_SKIP debug ablation: 1 attention, 2 sampler, 4 linears, 8 rope, 16 lm head
     // tcgen05 path: pre-split activation buffers, partial sums of squares, tensor maps
     bool tc_ok;
@@ -181,6 +182,7 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     sagc::g_pdl_all = m->use_pdl && env_int("SAGC_PDL_ALL", 1) != 0;
     m->gemv_max = env_int("SAGC_GEMV_MAX", 0);
     m->skip_mask = env_int("SAGC_SKIP", 0);
+    m->tc_min = env_int("SAGC_TC_MIN", 1);   // measured: the tcgen05 path beats the register-HMMA tail kernels at every batch size
     m->tok_buf = m->len_buf = m->forced_len_d = m->dump_list_d = m->prompt_tok_d = nullptr;
     m->tok_cap = m->forced_cap = m->dump_cap = m->prompt_cap = 0;
     m->row_cap = 0;
@@ -281,7 +283,7 @@ static int pick_kind(const sagc_model* m, int path, int m_max) {
     if (path == SAGC_PATH_GEMV) return LIN_GEMV;
     if (path == SAGC_PATH_GEMM) return m->tc_ok ? LIN_TC : LIN_MMA;
     if (m_max <= m->gemv_max) return LIN_GEMV;
-    if (m_max <= 8 || !m->tc_ok) return LIN_MMA;      // tail: register-resident HMMA kernel
+    if (m_max < m->tc_min || !m->tc_ok) return LIN_MMA;   // tail: register-resident HMMA kernel
     return LIN_TC;                                    // large batch / prefill: tcgen05 + TMEM
 }
 
