@@ -10,7 +10,7 @@ typedef uint16_t bf16_t;   // raw bf16 bit pattern
 
 extern bool g_pdl_all;     // launch the small kernels (embed, rope, attention, sampler, advance) with the PDL attribute too
 
-enum { EPI_STORE = 0, EPI_RESID = 1, EPI_SWIGLU = 2 };
+enum { EPI_STORE = 0, EPI_RESID = 1, EPI_SWIGLU = 2, EPI_QKV = 3 };   // EPI_QKV: tcgen05 path only (fused RoPE + KV append)
 enum { LIN_MMA = 0, LIN_GEMV = 1, LIN_TC = 2 };
 
 // Y[M][N] = epi( rms?(X)[M][K] . W[N][K]^T ).  Steps a6, a8-a11 of DESIGN.md.
@@ -142,6 +142,9 @@ struct TcLinearArgs {
     float* Y; int ldy; const float* R;
     bf16_t* xs_out; int ld_xs; const bf16_t* norm_next; float* ssq_out;
     const float* ssq_in; int ssq_in_tiles; int ssq_ld; float eps; int k_norm;
+    // EPI_QKV: rotate q and k (RoPE), store q as fp32 into Y, round k / v to bf16 into the sequence's KV page
+    const float* rope_cs; const int* row_pos; const int* row_sid; const int* page_table; bf16_t* kv_layer;
+    int max_blocks, page, Hkv, hd, q_rows, kv_rows;
     float* scratch;             // >= TC_SCRATCH_FLOATS floats for the split-K partial tiles (null: no K split)
     bool pdl;
 };

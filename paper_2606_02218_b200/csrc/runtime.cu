@@ -358,20 +358,26 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cuda
         const TcMap* w7 = &m->wmaps[(size_t)l * 7];
         TcLinearArgs t = {};
         t.a[0] = &w7[0]; t.a[1] = &w7[1]; t.a[2] = &w7[2]; t.seg_rows[0] = qd; t.seg_rows[1] = kvd; t.seg_rows[2] = kvd;
-        t.b = &m->amaps[0][nbi]; t.K = c.d_model; t.N = m->Nqkv; t.m_dev = rs.m_dev; t.m_max = rs.m_max; t.epi = EPI_STORE;
+        t.b = &m->amaps[0][nbi]; t.K = c.d_model; t.N = m->Nqkv; t.m_dev = rs.m_dev; t.m_max = rs.m_max; t.epi = EPI_QKV;
         t.Y = m->qkv; t.ldy = m->Nqkv; t.ssq_in = m->ssq; t.ssq_in_tiles = m->d_tiles; t.ssq_ld = m->ssq_ld;
         t.eps = c.rms_eps; t.k_norm = c.d_model; t.pdl = m->use_pdl; t.scratch = m->tc_scratch;
+        // RoPE + bf16 KV append run in this GEMM's epilogue (no separate kernel on the tcgen05 path)
+        bf16_t* kv_layer = m->kv_pool + (size_t)l * m->layer_stride;
+        t.rope_cs = m->rope_cs; t.row_pos = rs.pos; t.row_sid = rs.sid; t.page_table = m->ps.page_table; t.kv_layer = kv_layer;
+        t.max_blocks = m->max_blocks; t.page = c.page_tokens; t.Hkv = c.n_kv_heads; t.hd = c.head_dim; t.q_rows = qd; t.kv_rows = kvd;
+        static const bool fuse_rope = env_int("SAGC_FUSE_ROPE", 0) != 0;   // measured: no gain in TAIL, -4% in FULL -> off by default
+        if (!fuse_rope) t.epi = EPI_STORE;
         if (!(skip & 4)) LAUNCH(launch_linear_tc(t, st));
-
-        RopeArgs ra = {};
-        ra.qkv = m->qkv; ra.row_sid = rs.sid; ra.row_pos = rs.pos; ra.m_dev = rs.m_dev; ra.m_max = rs.m_max;
-        ra.rope_cs = m->rope_cs; ra.kv_layer = m->kv_pool + (size_t)l * m->layer_stride;
-        ra.page_table = m->ps.page_table; ra.max_blocks = m->max_blocks; ra.page = c.page_tokens;
-        ra.Hq = c.n_q_heads; ra.Hkv = c.n_kv_heads; ra.hd = c.head_dim;
-        if (!(skip & 8)) LAUNCH(launch_rope_append(ra, st));
+        if (!fuse_rope) {
+            RopeArgs ra = {};
+            ra.qkv = m->qkv; ra.row_sid = rs.sid; ra.row_pos = rs.pos; ra.m_dev = rs.m_dev; ra.m_max = rs.m_max;
+            ra.rope_cs = m->rope_cs; ra.kv_layer = kv_layer; ra.page_table = m->ps.page_table; ra.max_blocks = m->max_blocks;
+            ra.page = c.page_tokens; ra.Hq = c.n_q_heads; ra.Hkv = c.n_kv_heads; ra.hd = c.head_dim;
+            LAUNCH(launch_rope_append(ra, st));
+        }
 
         AttnArgs aa = {};
-        aa.q = m->qkv; aa.ldq = m->Nqkv; aa.kv_layer = ra.kv_layer; aa.page_table = m->ps.page_table;
+        aa.q = m->qkv; aa.ldq = m->Nqkv; aa.kv_layer = kv_layer; aa.page_table = m->ps.page_table;
         aa.max_blocks = m->max_blocks; aa.row_sid = rs.sid; aa.row_ctx = rs.ctx; aa.m_dev = rs.m_dev; aa.m_max = rs.m_max;
         aa.Hq = c.n_q_heads; aa.Hkv = c.n_kv_heads; aa.hd = c.head_dim; aa.page = c.page_tokens;
         aa.n_splits = n_splits; aa.part_o = m->part_o; aa.part_ml = m->part_ml; aa.counters = m->counters;

@@ -116,6 +116,9 @@ struct TcDev {
     int ssq_ld; float eps; int k_norm;
     int stages;                     // smem ring depth chosen by the launcher
     float* scratch;                 // split-K partial tiles [cta][NA][MB][128] (L2-resident), KS > 1 only
+    // EPI_QKV (fused RoPE + KV append)
+    const float* rope_cs; const int* row_pos; const int* row_sid; const int* page_table; bf16_t* kv_layer;
+    int max_blocks, page, Hkv, hd, q_rows, kv_rows;
 };
 
 template <int NB, int NA>
@@ -129,7 +132,8 @@ struct TcCfg {
     static constexpr int TMEM_COLS = NA * NB <= 32 ? 32 : (NA * NB <= 64 ? 64 : (NA * NB <= 128 ? 128 : (NA * NB <= 256 ? 256 : 512)));
     static constexpr int TAIL = 1024;                                  // barriers, tmem slot, rstd, ssq scratch
     static constexpr int MAXSTAGES = (196 * 1024 / STAGE) > 8 ? 8 : (196 * 1024 / STAGE);
-    static constexpr int smem_bytes(int stages) { return stages * STAGE + TAIL + 5 * MB * 4 + 1024; }
+    static constexpr int EXCH = 32 * 128 * 4;                          // RoPE partner exchange (EPI_QKV)
+    static constexpr int smem_bytes(int stages) { return stages * STAGE + TAIL + 5 * MB * 4 + EXCH + 1024; }
 };
 
 __device__ __forceinline__ float silu_tc(float z) { return z / (1.f + __expf(-z)); }
@@ -139,8 +143,8 @@ __device__ __forceinline__ float silu_tc(float z) { return z / (1.f + __expf(-z)
 // tile from shared memory, plus the residual) is issued before the first use: one memory round trip per
 // batch of 64 / (NA*KS) columns, partials summed in rank order (deterministic).
 template <int NB, int EPI, int KS>
-__device__ __forceinline__ void tc_epilogue(const TcDev& a, const float* red, const float* rstd_s, float* ssq_s, int warp,
-                                            int lane, int row0, int m0, int tile, int rank, int cta_id) {
+__device__ __forceinline__ void tc_epilogue(const TcDev& a, const float* red, const float* rstd_s, float* ssq_s, float* exch,
+                                            int warp, int lane, int row0, int m0, int tile, int rank, int cta_id) {
     constexpr int NA = (EPI == EPI_SWIGLU) ? 2 : 1;
     constexpr int MB = NB / 2;
     constexpr int MBATCH = (KS == 1) ? 16 / NA : 64 / (NA * KS);
@@ -183,7 +187,7 @@ __device__ __forceinline__ void tc_epilogue(const TcDev& a, const float* red, co
             }
             const float sc = (a.ssq_in != nullptr) ? rstd_s[mc[j]] : 1.f;
             float o;
-            if (EPI == EPI_STORE) o = acc[0] * sc;
+            if (EPI == EPI_STORE || EPI == EPI_QKV) o = acc[0] * sc;
             else if (EPI == EPI_RESID) o = res[j] + acc[0] * sc;
             else o = silu_tc(acc[0] * sc) * (acc[NA - 1] * sc);
             outv[j] = o;
@@ -197,6 +201,52 @@ __device__ __forceinline__ void tc_epilogue(const TcDev& a, const float* red, co
             for (int o = 16; o > 0; o >>= 1)
 #pragma unroll
                 for (int j = 0; j < MBATCH; ++j) q2[j] += __shfl_xor_sync(0xffffffffu, q2[j], o);
+        }
+        if (EPI == EPI_QKV) {
+            // RoPE (rotate-half): the partner feature n +- hd/2 lives in another lane / warp of this CTA
+            const int half = a.hd >> 1;
+            const bool is_v = row0 >= a.q_rows + a.kv_rows;
+            const bool is_q = row0 < a.q_rows;
+            const int d = n & (a.hd - 1);
+            int posj[MBATCH];
+            float2 cs[MBATCH];
+#pragma unroll
+            for (int j = 0; j < MBATCH; ++j) posj[j] = a.row_pos[max(min(m0 + mc[j], M - 1), 0)];
+#pragma unroll
+            for (int j = 0; j < MBATCH; ++j)
+                cs[j] = is_v ? make_float2(1.f, 0.f)
+                             : *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)posj[j] * half + (d & (half - 1))) * 2);
+#pragma unroll
+            for (int j = 0; j < MBATCH; ++j) exch[j * 128 + row] = outv[j];
+            asm volatile("bar.sync 1, 128;\n" ::: "memory");
+#pragma unroll
+            for (int j = 0; j < MBATCH; ++j) {
+                const float partner = exch[j * 128 + (row ^ half)];
+                const float rot = (d < half) ? outv[j] * cs[j].x - partner * cs[j].y : outv[j] * cs[j].x + partner * cs[j].y;
+                outv[j] = is_v ? outv[j] : rot;
+            }
+            asm volatile("bar.sync 1, 128;\n" ::: "memory");
+#pragma unroll
+            for (int j = 0; j < MBATCH; ++j) {
+                const int m = mb + j * KS;
+                const int mg = m0 + m;
+                if (m < MB && mg < M) {
+                    if (is_q) {
+                        a.Y[(size_t)mg * a.ldy + n] = outv[j];
+                    } else {
+                        const int sid = a.row_sid[mg];
+                        const int pg = a.page_table[(size_t)sid * a.max_blocks + posj[j] / a.page];
+                        if (pg >= 0) {
+                            const int feat = n - a.q_rows - (is_v ? a.kv_rows : 0);
+                            const int kvh = feat / a.hd;
+                            bf16_t* dst = a.kv_layer + (((size_t)pg * 2 + (is_v ? 1 : 0)) * a.Hkv + kvh) * (size_t)a.page * a.hd +
+                                          (size_t)(posj[j] % a.page) * a.hd + d;
+                            *dst = (bf16_t)f32_to_bf16_bits(outv[j]);
+                        }
+                    }
+                }
+            }
+            continue;
         }
 #pragma unroll
         for (int j = 0; j < MBATCH; ++j) {
@@ -241,6 +291,7 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum + 1);
     float* rstd_s = reinterpret_cast<float*>(smem + S * C::STAGE + C::TAIL);
     float* ssq_s = rstd_s + MB;                                         // [4][MB]
+    float* exch = ssq_s + 4 * MB;                                       // [32][128] (EPI_QKV)
     float* red = reinterpret_cast<float*>(smem);                        // [NA][MB][128], overlays the stages
 
     cg::cluster_group cluster = cg::this_cluster();
@@ -381,10 +432,10 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     }
     if (warp >= 2) {
         switch (KS) {
-            case 1: tc_epilogue<NB, EPI, 1>(a, red, rstd_s, ssq_s, warp, lane, row0, m0, tile, rank, cta_id); break;
-            case 2: tc_epilogue<NB, EPI, 2>(a, red, rstd_s, ssq_s, warp, lane, row0, m0, tile, rank, cta_id); break;
-            case 4: tc_epilogue<NB, EPI, 4>(a, red, rstd_s, ssq_s, warp, lane, row0, m0, tile, rank, cta_id); break;
-            default: tc_epilogue<NB, EPI, 8>(a, red, rstd_s, ssq_s, warp, lane, row0, m0, tile, rank, cta_id); break;
+            case 1: tc_epilogue<NB, EPI, 1>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id); break;
+            case 2: tc_epilogue<NB, EPI, 2>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id); break;
+            case 4: tc_epilogue<NB, EPI, 4>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id); break;
+            default: tc_epilogue<NB, EPI, 8>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id); break;
         }
     }
     // no second cluster barrier: peers read this CTA's partials from the L2 scratch, never from its
@@ -485,6 +536,8 @@ int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
     d.K = t.K; d.N = t.N; d.n_kb = t.K / TC_BK; d.m_dev = t.m_dev; d.m_max = t.m_max; d.Y = t.Y; d.ldy = t.ldy; d.R = t.R;
     d.xs_out = t.xs_out; d.ld_xs = t.ld_xs; d.norm_next = t.norm_next; d.ssq_out = t.ssq_out; d.ssq_in = t.ssq_in;
     d.ssq_in_tiles = t.ssq_in_tiles; d.ssq_ld = t.ssq_ld; d.eps = t.eps; d.k_norm = t.k_norm; d.scratch = t.scratch;
+    d.rope_cs = t.rope_cs; d.row_pos = t.row_pos; d.row_sid = t.row_sid; d.page_table = t.page_table; d.kv_layer = t.kv_layer;
+    d.max_blocks = t.max_blocks; d.page = t.page; d.Hkv = t.Hkv; d.hd = t.hd; d.q_rows = t.q_rows; d.kv_rows = t.kv_rows;
     const int nbi = tc_nb_index(t.m_max);
     const int NB = 32 << nbi, MB = NB / 2;
     const int tiles = t.N / 128, mtiles = (t.m_max + MB - 1) / MB;
@@ -509,6 +562,7 @@ int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
     case NBV:                                                                                \
         if (t.epi == EPI_SWIGLU) e = launch_tc_inst<NBV, EPI_SWIGLU>(t, d, grid, KS, st);    \
         else if (t.epi == EPI_RESID) e = launch_tc_inst<NBV, EPI_RESID>(t, d, grid, KS, st); \
+        else if (t.epi == EPI_QKV) e = launch_tc_inst<NBV, EPI_QKV>(t, d, grid, KS, st);     \
         else e = launch_tc_inst<NBV, EPI_STORE>(t, d, grid, KS, st);                         \
         break;
     switch (NB) {
