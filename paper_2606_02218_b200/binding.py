@@ -15,7 +15,7 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libsagc.so")
+LIB_PATH = os.environ.get("SAGC_LIB", os.path.join(_HERE, "libsagc.so"))   # SAGC_LIB: A/B a differently built library
 
 OK, EINVAL, ENOMEM, EPAGES, ECUDA = 0, -1, -2, -3, -4
 MODE_GREEDY, MODE_GUMBEL = 0, 1

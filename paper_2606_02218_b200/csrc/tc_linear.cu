@@ -144,16 +144,13 @@ __device__ __forceinline__ float silu_tc(float z) { return z / (1.f + __expf(-z)
 // batch of 64 / (NA*KS) columns, partials summed in rank order (deterministic).
 template <int NB, int EPI, int KS>
 __device__ __forceinline__ void tc_epilogue(const TcDev& a, const float* red, const float* rstd_s, float* ssq_s, float* exch,
-                                            int warp, int lane, int row0, int m0, int tile, int rank, int cta_id) {
+                                            int warp, int lane, int row0, int m0, int tile, int rank, int cta_id, int M, float nw) {
     constexpr int NA = (EPI == EPI_SWIGLU) ? 2 : 1;
     constexpr int MB = NB / 2;
     constexpr int MBATCH = (KS == 1) ? 16 / NA : 64 / (NA * KS);
-    const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
     const int lg = warp & 3;
     const int row = lg * 32 + lane;
     const int n = row0 + row;
-    float nw = 1.f;
-    if (EPI == EPI_RESID && a.norm_next != nullptr) nw = bf16_to_f32(a.norm_next[n]);
     const float* base = (KS == 1) ? red : a.scratch + (size_t)(cta_id - rank) * (NA * MB * 128);
     for (int mb = rank; mb < MB; mb += KS * MBATCH) {
         if (m0 + mb >= M) break;
@@ -327,6 +324,8 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
+    int M_pre = a.m_max;
+    float nw_pre = 1.f;
     if (warp == 0) {
         // ===== TMA producer =====
         if (lane == 0) {
@@ -381,10 +380,14 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         }
     } else {
         // ===== epilogue warps: TMEM -> (hi + lo) -> shared reduce buffer =====
-        pdl_wait();
-        pdl_launch();
         const int lg = warp & 3;                      // TMEM lane group of this warp
         const int row = lg * 32 + lane;
+        // everything the final epilogue needs that does not depend on the accumulator is fetched now,
+        // off the critical path: the next norm's gain (a weight: even before the dependency wait) and the live count
+        if (EPI == EPI_RESID && a.norm_next != nullptr) nw_pre = bf16_to_f32(a.norm_next[row0 + row]);
+        pdl_wait();
+        pdl_launch();
+        M_pre = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
         const int et = (warp - 2) * 32 + lane;        // 0..127
         if (a.ssq_in != nullptr) {
             for (int m = et; m < MB; m += 128) {
@@ -432,10 +435,10 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     }
     if (warp >= 2) {
         switch (KS) {
-            case 1: tc_epilogue<NB, EPI, 1>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id); break;
-            case 2: tc_epilogue<NB, EPI, 2>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id); break;
-            case 4: tc_epilogue<NB, EPI, 4>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id); break;
-            default: tc_epilogue<NB, EPI, 8>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id); break;
+            case 1: tc_epilogue<NB, EPI, 1>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id, M_pre, nw_pre); break;
+            case 2: tc_epilogue<NB, EPI, 2>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id, M_pre, nw_pre); break;
+            case 4: tc_epilogue<NB, EPI, 4>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id, M_pre, nw_pre); break;
+            default: tc_epilogue<NB, EPI, 8>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id, M_pre, nw_pre); break;
         }
     }
     // no second cluster barrier: peers read this CTA's partials from the L2 scratch, never from its
