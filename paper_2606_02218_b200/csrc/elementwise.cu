@@ -35,21 +35,30 @@ int launch_embed(const bf16_t* embed, const int* tok, const int* m_dev, int m_ma
 // and written to slot pos%page of page page_table[sid][pos/page] -- the ONLY rounding point of
 // the forward pass (reading C1).  grid = (rows, Hq+2*Hkv heads), block = hd/2 threads.
 __global__ void k_rope_append(RopeArgs a) {
-    trace_mark(8); pdl_wait(); trace_mark(9);
-    pdl_launch();
+    trace_mark(8);
+    // Positions, the live count, the page table and the RoPE table were written by EARLIER steps (or are
+    // constants): fetch them before the dependency wait so that only the q/k/v loads remain after it.
     const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
     const int row = blockIdx.x;
-    if (row >= M) return;
     const int head = blockIdx.y;
     const int half = a.hd >> 1;
     const int i = threadIdx.x;
-    if (i >= half) return;
-    const int pos = a.row_pos[row];
+    const bool live = row < M && i < half;
+    int pos = 0, pg = -1;
+    float2 cs = make_float2(1.f, 0.f);
+    if (live) {
+        pos = a.row_pos[row];
+        if (head < a.Hq + a.Hkv) cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)pos * half + i) * 2);
+        if (head >= a.Hq) pg = a.page_table[(size_t)a.row_sid[row] * a.max_blocks + pos / a.page];
+    }
+    pdl_wait();
+    trace_mark(9);
+    pdl_launch();
+    if (!live) return;
     const int ld = (a.Hq + 2 * a.Hkv) * a.hd;
     float* hp = a.qkv + (size_t)row * ld + (size_t)head * a.hd;
     float x0 = hp[i], x1 = hp[i + half];
     if (head < a.Hq + a.Hkv) {
-        const float2 cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)pos * half + i) * 2);
         float r0 = x0 * cs.x - x1 * cs.y;
         float r1 = x1 * cs.x + x0 * cs.y;
         x0 = r0; x1 = r1;
@@ -58,8 +67,6 @@ __global__ void k_rope_append(RopeArgs a) {
         hp[i] = x0; hp[i + half] = x1;
         return;
     }
-    const int sid = a.row_sid[row];
-    const int pg = a.page_table[(size_t)sid * a.max_blocks + pos / a.page];
     if (pg < 0) return;   // unmapped (only after a pool-exhaustion error)
     const int isv = head >= a.Hq + a.Hkv;
     const int kvh = head - a.Hq - (isv ? a.Hkv : 0);
