@@ -501,7 +501,9 @@ static cudaError_t launch_tc_inst(const TcLinearArgs& t, const TcDev& d, dim3 gr
     // grids that fit the chip in one wave get the deepest ring; multi-wave grids (LM head, prefill) keep
     // ~100 KB so two CTAs share an SM and one's epilogue overlaps the other's loads
     const bool one_wave = (long long)grid.x * grid.y * grid.z <= 148;
-    const int stages = one_wave ? C::MAXSTAGES : C::STAGES;
+    // wide batch tiles (UMMA N = 256) are throughput-bound per CTA: give them the deepest ring as well
+    static const int deep256 = [] { const char* e = getenv("SAGC_TC_DEEP256"); return e ? atoi(e) : 1; }();
+    const int stages = (one_wave || (NB == 256 && deep256)) ? C::MAXSTAGES : C::STAGES;
     const int smem = C::smem_bytes(stages);
     TcDev d2 = d; d2.stages = stages;
     static bool attr_set = false;
