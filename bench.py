@@ -267,10 +267,11 @@ def main():
     achieved = dec_bytes / dec_ms / 1e6
     line = {"metric": METRIC, "value": world * acc["tokens"] / ms * 1e3, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "bf16 weights/KV, fp32 activations+accumulate", "data": "synthetic",
+            "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": f"configs[{args.cfg - 1}]: 0.5B-shaped decoder, {w.n_prompts} prompts x {w.prompt_len} tokens x G={w.G}, "
                                    f"forced lengths lognormal(median 1024, sigma 0.8) cap {max_new}, Gumbel T=1 Philox",
-                       "tokens_per_step": acc["tokens"] // args.steps, "l2": "weights 0.99 GB per decode step > 126 MB L2",
+                       "tokens_per_step": acc["tokens"] // args.steps,
+                       "precision": "bf16 weights and KV cache, activations carried as hi+lo bf16 pairs (~16 mantissa bits), fp32 accumulate", "l2": "weights 0.99 GB per decode step > 126 MB L2",
                        "replicas": world},
             "clocks": clocks, "gpu_launches": acc["launches"],
             "e2e": {"value": world * e2e_tok / e2e_ms * 1e3, "unit": UNIT, "h2d_bytes_per_step": int(prompts.nbytes + fl.nbytes),

@@ -288,3 +288,26 @@ def test_config4_truncated(B, cfg, G):
     then the tail path; logits of two sampled sequences against the fp32 oracle."""
     fl = np.array([6, 4, 6, 3, 6, 2, 6, 1, 6, 4, 6, 3] + [1, 2, 3, 4] * 5, dtype=np.int32)   # 6 live in steps 5-6
     _sampled_parity(B, cfg, 1, 128, G, 6, fl, 0, n_dump_seq=2)
+
+
+def test_variable_G_per_call_same_handle(B):
+    """Config 4's pattern: the controller re-chooses G every rollout step; one handle, a seeded G schedule,
+    per-step Philox seed = base + step.  Every call must match the oracle exactly (tiny model)."""
+    w = wl.tiny_variant(1, n_prompts=2)
+    weights = wl.make_weights(w.model, 0)
+    prompts, offs = wl.make_prompts(w, n_prompts=2, prompt_len=24)       # ragged vs the 16-token page
+    dec = odec.RefDecoder(w.model, weights)
+    m = B.Model(w.model, weights, 400, 2 * 16, 24 + 20)
+    rng = np.random.default_rng(4)
+    for step, G in enumerate([4, 8, 16, 8, 4]):
+        fl = rng.integers(1, 21, size=2 * G).astype(np.int32)
+        seed = 4004 + step
+        ref = oro.rollout_group(dec, prompts, offs, G, 1, 1.0, seed, 20, forced_lengths=fl, n_pages=400, page_tokens=16)
+        out = m.rollout_group(prompts, offs, G, mode=B.MODE_GUMBEL, temperature=1.0, seed=seed, max_new_tokens=20,
+                              forced_lengths=fl, flags=B.FLAG_LOG)
+        _check_structure(B, m, ref.paging, out, ref.lengths)
+        toks = out.tokens.cpu().numpy()
+        n_bad, n_dis, n_all = _token_rule(dec, 1, 1.0, seed, prompts, offs, G, toks, ref.lengths)
+        assert n_bad == 0 and n_dis <= max(1, 0.005 * n_all), (step, G, n_bad, n_dis, n_all)
+        assert np.array_equal(out.len_stats.cpu().numpy(), ref.len_stats)
+    m.close()
