@@ -127,6 +127,22 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
             cp_async16(base + (size_t)(ATT_TILE + j) * ROWB + ((part ^ vsw(j)) << 4), vp, ok ? 16 : 0);
         }
     };
+    // fused RoPE (decode): cos/sin of this row's position for the q fragments, fetched before the wait
+    const bool fuse = a.fuse_rope != 0;
+    float2 qcs[(KB / 2 > 0 ? KB / 2 : 1)][8];
+    int pos_new = 0;
+    if (fuse) {
+        pos_new = a.row_pos[row];
+#pragma unroll
+        for (int kb = 0; kb < KB / 2; ++kb)
+#pragma unroll
+            for (int e = 0; e < 8; ++e)
+                qcs[kb][e] = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)pos_new * (HD / 2) + kb * 32 + 8 * q + e) * 2);
+    }
+    // the split that holds the newest position appends its K,V (rotated, rounded to bf16)
+    const bool designated = fuse && n_tiles > 0 && t_end == ctx;
+    float2 kcs = make_float2(1.f, 0.f);
+    if (designated && tid < HD / 2) kcs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)pos_new * (HD / 2) + tid) * 2);
     // tiles that do not contain the newest position (ctx - 1) can be fetched before the wait
     const bool early0 = a.prefetch && n_tiles > 0 && (t_begin + ATT_TILE <= ctx - 1);
     const bool early1 = early0 && n_tiles > 1 && (t_begin + 2 * ATT_TILE <= ctx - 1);
@@ -142,9 +158,11 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
 
     // Q fragments (hi in rows g, lo in rows g+8), pre-scaled by 1/sqrt(hd); head g of this kv head
     uint32_t qf[KB][8];
+    uint32_t knew = 0, vnew = 0;                    // designated CTA: bf16 bits of the new k pair / v element
     {
         const float scale = rsqrtf((float)HD);
         const float* qp = a.q + (size_t)row * a.ldq + (size_t)(kvh * r + g) * HD + 8 * q;
+        float xq[KB][8];
 #pragma unroll
         for (int kb = 0; kb < KB; ++kb) {
             float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0;
@@ -152,10 +170,47 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
                 x0 = *reinterpret_cast<const float4*>(qp + kb * 32);
                 x1 = *reinterpret_cast<const float4*>(qp + kb * 32 + 4);
             }
-            split2(x0.x * scale, x0.y * scale, qf[kb][0], qf[kb][4]);
-            split2(x0.z * scale, x0.w * scale, qf[kb][1], qf[kb][5]);
-            split2(x1.x * scale, x1.y * scale, qf[kb][2], qf[kb][6]);
-            split2(x1.z * scale, x1.w * scale, qf[kb][3], qf[kb][7]);
+            xq[kb][0] = x0.x; xq[kb][1] = x0.y; xq[kb][2] = x0.z; xq[kb][3] = x0.w;
+            xq[kb][4] = x1.x; xq[kb][5] = x1.y; xq[kb][6] = x1.z; xq[kb][7] = x1.w;
+        }
+        if (designated) {
+            // raw k (pair i, i + hd/2) and v of the newest position from the same qkv row
+            const float* kp = a.q + (size_t)row * a.ldq + (size_t)a.Hq * HD + (size_t)kvh * HD;
+            const float* vp = kp + (size_t)a.Hkv * HD;
+            if (tid < HD / 2) {
+                const float k0 = kp[tid], k1 = kp[tid + HD / 2];
+                knew = f32_to_bf16_bits(k0 * kcs.x - k1 * kcs.y) | (f32_to_bf16_bits(k1 * kcs.x + k0 * kcs.y) << 16);
+            }
+            if (tid < HD) vnew = f32_to_bf16_bits(vp[tid]);
+        }
+        if (fuse) {
+#pragma unroll
+            for (int kb = 0; kb < KB / 2; ++kb)
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const float lo = xq[kb][e], hi = xq[kb + KB / 2][e];
+                    xq[kb][e] = lo * qcs[kb][e].x - hi * qcs[kb][e].y;
+                    xq[kb + KB / 2][e] = hi * qcs[kb][e].x + lo * qcs[kb][e].y;
+                }
+        }
+#pragma unroll
+        for (int kb = 0; kb < KB; ++kb) {
+            split2(xq[kb][0] * scale, xq[kb][1] * scale, qf[kb][0], qf[kb][4]);
+            split2(xq[kb][2] * scale, xq[kb][3] * scale, qf[kb][1], qf[kb][5]);
+            split2(xq[kb][4] * scale, xq[kb][5] * scale, qf[kb][2], qf[kb][6]);
+            split2(xq[kb][6] * scale, xq[kb][7] * scale, qf[kb][3], qf[kb][7]);
+        }
+        if (designated) {
+            // append to the page (for the later steps); this step's copy is patched into shared memory below
+            const int tnew = ctx - 1;
+            const int blk = tnew >> pshift;
+            const int pg = pg_cached ? pg_s[blk - b_begin] : pt[blk];
+            if (pg >= 0) {
+                bf16_t* kd = a.kv_layer_w + ((size_t)pg * 2 * a.Hkv + kvh) * head_stride + (size_t)(tnew & pmask) * HD;
+                bf16_t* vd = kd + (size_t)a.Hkv * head_stride;
+                if (tid < HD / 2) { kd[tid] = (bf16_t)(knew & 0xffffu); kd[tid + HD / 2] = (bf16_t)(knew >> 16); }
+                if (tid < HD) vd[tid] = (bf16_t)vnew;
+            }
         }
     }
     float o[NT][4];
@@ -172,6 +227,19 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
         if (tile == 0) trace_mark(10 * 4 + 1);                         // tile landed; the stage of tile-1 is free
         if (tile + 2 < n_tiles) load_tile(tile + 2, (tile + 2) % ATT_STAGES);
         cp_async_commit();
+        if (designated && tile == n_tiles - 1) {
+            // the row of the newest position was copied stale from the page: overwrite it with the new K,V
+            unsigned char* sb = kv_s + (size_t)(tile % ATT_STAGES) * AttSmem<HD>::STAGE;
+            const int j = (ctx - 1) - (t_begin + tile * ATT_TILE);
+            if (tid < HD / 2) {
+                const int d0 = tid, d1 = tid + HD / 2;
+                *reinterpret_cast<bf16_t*>(sb + (size_t)j * ROWB + (((d0 >> 3) ^ ksw(j)) << 4) + (d0 & 7) * 2) = (bf16_t)(knew & 0xffffu);
+                *reinterpret_cast<bf16_t*>(sb + (size_t)j * ROWB + (((d1 >> 3) ^ ksw(j)) << 4) + (d1 & 7) * 2) = (bf16_t)(knew >> 16);
+            }
+            if (tid < HD)
+                *reinterpret_cast<bf16_t*>(sb + (size_t)(ATT_TILE + j) * ROWB + (((tid >> 3) ^ vsw(j)) << 4) + (tid & 7) * 2) = (bf16_t)vnew;
+            __syncthreads();
+        }
         const unsigned char* kbase = kv_s + (size_t)(tile % ATT_STAGES) * AttSmem<HD>::STAGE;
         const unsigned char* vbase = kbase + (size_t)ATT_TILE * ROWB;
         const int tw = warp * 16;                // this warp's 16 tokens inside the tile

@@ -66,6 +66,9 @@ struct AttnArgs {
     float* out;             // [M][Hq*hd] fp32 (used when out_split is null)
     bf16_t* out_split;      // pre-split rows [2m] = hi, [2m+1] = lo, row stride ld_split (tcgen05 path)
     int ld_split;
+    // decode only (fuse_rope): q is the RAW qkv row; RoPE of q / k and the bf16 K,V append of the newest
+    // position happen inside this kernel (no separate RoPE kernel).  head_dim >= 64.
+    int fuse_rope; const float* rope_cs; const int* row_pos; bf16_t* kv_layer_w;
     int prefetch;           // 1 in decode: cached positions older than the newest one predate the upstream kernel
 };
 int launch_attention(const AttnArgs& a, cudaStream_t st);

@@ -368,7 +368,10 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cuda
         static const bool fuse_rope = env_int("SAGC_FUSE_ROPE", 0) != 0;   // measured: no gain in TAIL, -4% in FULL -> off by default
         if (!fuse_rope) t.epi = EPI_STORE;
         if (!(skip & 4)) LAUNCH(launch_linear_tc(t, st));
-        if (!fuse_rope) {
+        // decode: RoPE + KV append are done inside the attention kernel (one launch less per layer)
+        static const bool fuse_att_env = env_int("SAGC_FUSE_ATT", 1) != 0;
+        const bool fuse_att = fuse_att_env && !fuse_rope && rs.m_dev != nullptr && c.head_dim >= 64;
+        if (!fuse_rope && !fuse_att) {
             RopeArgs ra = {};
             ra.qkv = m->qkv; ra.row_sid = rs.sid; ra.row_pos = rs.pos; ra.m_dev = rs.m_dev; ra.m_max = rs.m_max;
             ra.rope_cs = m->rope_cs; ra.kv_layer = kv_layer; ra.page_table = m->ps.page_table; ra.max_blocks = m->max_blocks;
@@ -382,6 +385,7 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cuda
         aa.Hq = c.n_q_heads; aa.Hkv = c.n_kv_heads; aa.hd = c.head_dim; aa.page = c.page_tokens;
         aa.n_splits = n_splits; aa.part_o = m->part_o; aa.part_ml = m->part_ml; aa.counters = m->counters;
         aa.out = m->att; aa.prefetch = (rs.m_dev != nullptr) ? 1 : 0; aa.out_split = m->att_s; aa.ld_split = qd;
+        aa.fuse_rope = fuse_att ? 1 : 0; aa.rope_cs = m->rope_cs; aa.row_pos = rs.pos; aa.kv_layer_w = kv_layer;
         if (!(skip & 1)) LAUNCH(launch_attention(aa, st));
 
         TcLinearArgs o = {};
