@@ -311,3 +311,21 @@ def test_variable_G_per_call_same_handle(B):
         assert n_bad == 0 and n_dis <= max(1, 0.005 * n_all), (step, G, n_bad, n_dis, n_all)
         assert np.array_equal(out.len_stats.cpu().numpy(), ref.len_stats)
     m.close()
+
+
+def test_no_graph_flag_gives_identical_tokens(B):
+    """SAGC_FLAG_NO_GRAPH launches the same kernels directly: tokens, lengths and page state must not change."""
+    w = wl.tiny_variant(1, model_n_q_heads=4, model_n_kv_heads=2, model_head_dim=64, model_d_model=256,
+                        model_d_ff=512, model_n_layers=2, model_vocab=1024, model_page_tokens=16)
+    weights = wl.make_weights(w.model, 3)
+    prompts, offs = wl.make_prompts(w, n_prompts=2, prompt_len=20)
+    fl = np.array([9, 30, 30, 2, 17, 30], dtype=np.int32)
+    m = B.Model(w.model, weights, 100, 6, 20 + 30)
+    outs = []
+    for flags in (B.FLAG_LOG, B.FLAG_LOG | B.FLAG_NO_GRAPH):
+        out = m.rollout_group(prompts, offs, 3, mode=B.MODE_GUMBEL, temperature=0.9, seed=11, max_new_tokens=30,
+                              forced_lengths=fl, flags=flags)
+        outs.append((out.tokens.cpu().numpy(), out.lengths.cpu().numpy(), m.debug_page_table(), m.debug_alloc_log()))
+    for a, b in zip(outs[0], outs[1]):
+        assert np.array_equal(a, b)
+    m.close()
