@@ -133,7 +133,9 @@ struct TcCfg {
     static constexpr int TAIL = 1024;                                  // barriers, tmem slot, rstd, ssq scratch
     static constexpr int MAXSTAGES = (196 * 1024 / STAGE) > 8 ? 8 : (196 * 1024 / STAGE);
     static constexpr int EXCH = 32 * 128 * 4;                          // RoPE partner exchange (EPI_QKV)
-    static constexpr int smem_bytes(int stages) { return stages * STAGE + TAIL + 5 * MB * 4 + EXCH + 1024; }
+    // the exchange buffer exists only in the EPI_QKV instantiation: 16 KB more would cost the SwiGLU kernel its
+    // second CTA per SM (152 CTAs -> two waves)
+    static constexpr int smem_bytes(int stages, bool qkv) { return stages * STAGE + TAIL + 5 * MB * 4 + (qkv ? EXCH : 0) + 1024; }
 };
 
 __device__ __forceinline__ float silu_tc(float z) { return z / (1.f + __expf(-z)); }
@@ -504,11 +506,12 @@ static cudaError_t launch_tc_inst(const TcLinearArgs& t, const TcDev& d, dim3 gr
     // wide batch tiles (UMMA N = 256) are throughput-bound per CTA: give them the deepest ring as well
     static const int deep256 = [] { const char* e = getenv("SAGC_TC_DEEP256"); return e ? atoi(e) : 1; }();
     const int stages = (one_wave || (NB == 256 && deep256)) ? C::MAXSTAGES : C::STAGES;
-    const int smem = C::smem_bytes(stages);
+    const int smem = C::smem_bytes(stages, EPI == EPI_QKV);
     TcDev d2 = d; d2.stages = stages;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_linear_tc<NB, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::smem_bytes(C::MAXSTAGES));
+        cudaError_t e = cudaFuncSetAttribute(k_linear_tc<NB, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::smem_bytes(C::MAXSTAGES, EPI == EPI_QKV));
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
