@@ -561,6 +561,8 @@ int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
     if (KS < 1) KS = 1;
     if (KS > 8) KS = 8;
     if (KS > d.n_kb) KS = d.n_kb;
+    static const int ks_swiglu = [] { const char* e = getenv("SAGC_TC_KS_SWIGLU"); return e ? atoi(e) : 0; }();
+    if (t.epi == EPI_SWIGLU && ks_swiglu > 0 && tiles * mtiles * ks_swiglu <= 2 * 148) KS = ks_swiglu;   // scratch holds 296 CTA tiles
     if (t.scratch == nullptr) KS = 1;
     { int p2 = 1; while (p2 * 2 <= KS) p2 *= 2; KS = p2; }      // the epilogue is specialised for 1, 2, 4, 8
     d.kb_per_cta = (d.n_kb + KS - 1) / KS;             // trailing ranks may get fewer (or zero) k blocks
