@@ -2,8 +2,8 @@
 //
 // One CTA per (activation row, kv head, K-split).  The r = Hq/Hkv query heads that share a kv
 // head are processed together so every K/V byte is read once per (row, kv head).  Contexts are
-// walked through the page table in tiles of 64 tokens, staged in shared memory by a 3-stage
-// cp.async pipeline (K and V rows, padded so that per-token 16-byte reads are conflict-free):
+// walked through the page table in tiles of 64 tokens, staged in shared memory by a 3/4-stage
+// cp.async pipeline (K and V rows, 16-byte chunks XOR-swizzled so that fragment reads are conflict-free):
 //   phase 1  thread = token: s[h] = q[h] . k  for the r heads (q pre-scaled, fp32, smem broadcast)
 //   softmax  online (running max / sum per head), warp-shuffle reductions, probabilities in smem
 //   phase 2  thread = (token group, 4 head-dim columns): o[h][:] += p[h][tok] * v[tok][:]
@@ -17,7 +17,6 @@ namespace sagc {
 
 static constexpr int ATT_THREADS = 128;
 static constexpr int ATT_TILE = 64;          // tokens per pipeline stage
-static constexpr int ATT_STAGES = 3;
 static constexpr int ATT_MAXR = 8;
 static constexpr int ATT_MAXPG = 1104;       // page ids cached per split (17408 / 16 + slack)
 
@@ -44,7 +43,8 @@ template <int HD>
 struct AttSmem {
     static constexpr int ROWB = HD * 2;                       // unpadded rows, 16-byte chunks XOR-swizzled
     static constexpr int STAGE = 2 * ATT_TILE * ROWB;         // K rows then V rows
-    static constexpr int BYTES = ATT_STAGES * STAGE;
+    static constexpr int NSTAGE = HD >= 128 ? 3 : 4;           // K/V tiles in flight: NSTAGE - 1 (<= ~100 KB per CTA)
+    static constexpr int BYTES = NSTAGE * STAGE;
 };
 
 __device__ __forceinline__ void ldmatrix_x4_trans(uint32_t (&r)[4], const void* smem_row) {
@@ -66,6 +66,7 @@ __device__ __forceinline__ void ldmatrix_x4_trans(uint32_t (&r)[4], const void* 
 template <int HD>
 __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     constexpr int ROWB = AttSmem<HD>::ROWB;
+    constexpr int ATT_STAGES = AttSmem<HD>::NSTAGE;
     constexpr int CPR = HD * 2 / 16;            // 16-byte chunks per row
     constexpr int KB = HD / 32;                 // 32-wide d blocks
     constexpr int NT = HD / 8;                  // output n-tiles
@@ -144,17 +145,16 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     float2 kcs = make_float2(1.f, 0.f);
     if (designated && tid < HD / 2) kcs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)pos_new * (HD / 2) + tid) * 2);
     // tiles that do not contain the newest position (ctx - 1) can be fetched before the wait
-    const bool early0 = a.prefetch && n_tiles > 0 && (t_begin + ATT_TILE <= ctx - 1);
-    const bool early1 = early0 && n_tiles > 1 && (t_begin + 2 * ATT_TILE <= ctx - 1);
-    if (early0) load_tile(0, 0);
-    if (early0) cp_async_commit();
-    if (early1) load_tile(1, 1);
-    if (early1) cp_async_commit();
+    // leading tiles that hold only positions older than ctx - 1 (at most ATT_STAGES - 1 of them)
+    int n_early = 0;
+    if (a.prefetch) {
+        while (n_early < ATT_STAGES - 1 && n_early < n_tiles && t_begin + (n_early + 1) * ATT_TILE <= ctx - 1) ++n_early;
+    }
+    for (int s2 = 0; s2 < n_early; ++s2) { load_tile(s2, s2); cp_async_commit(); }
     if (a.prefetch) pdl_wait();
     trace_mark(13);
     pdl_launch();
-    if (!early0) { if (n_tiles > 0) load_tile(0, 0); cp_async_commit(); }
-    if (!early1) { if (n_tiles > 1) load_tile(1, 1); cp_async_commit(); }
+    for (int s2 = n_early; s2 < ATT_STAGES - 1; ++s2) { if (s2 < n_tiles) load_tile(s2, s2); cp_async_commit(); }
 
     // Q fragments (hi in rows g, lo in rows g+8), pre-scaled by 1/sqrt(hd); head g of this kv head
     uint32_t qf[KB][8];
@@ -222,10 +222,10 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
 
     trace_mark(10 * 4 + 0);
     for (int tile = 0; tile < n_tiles; ++tile) {
-        cp_async_wait<1>();
+        cp_async_wait<ATT_STAGES - 2>();
         __syncthreads();
         if (tile == 0) trace_mark(10 * 4 + 1);                         // tile landed; the stage of tile-1 is free
-        if (tile + 2 < n_tiles) load_tile(tile + 2, (tile + 2) % ATT_STAGES);
+        if (tile + ATT_STAGES - 1 < n_tiles) load_tile(tile + ATT_STAGES - 1, (tile + ATT_STAGES - 1) % ATT_STAGES);
         cp_async_commit();
         if (designated && tile == n_tiles - 1) {
             // the row of the newest position was copied stale from the page: overwrite it with the new K,V
