@@ -43,7 +43,7 @@ template <int HD>
 struct AttSmem {
     static constexpr int ROWB = HD * 2;                       // unpadded rows, 16-byte chunks XOR-swizzled
     static constexpr int STAGE = 2 * ATT_TILE * ROWB;         // K rows then V rows
-    static constexpr int NSTAGE = HD >= 128 ? 3 : 4;           // K/V tiles in flight: NSTAGE - 1 (<= ~100 KB per CTA)
+    static constexpr int NSTAGE = HD >= 128 ? 3 : 6;           // K/V tiles in flight: NSTAGE - 1 (<= ~100 KB per CTA)
     static constexpr int BYTES = NSTAGE * STAGE;
 };
 
