@@ -2,7 +2,7 @@
 //
 // One CTA per (activation row, kv head, K-split).  The r = Hq/Hkv query heads that share a kv
 // head are processed together so every K/V byte is read once per (row, kv head).  Contexts are
-// walked through the page table in tiles of 64 tokens, staged in shared memory by a 3/4-stage
+// walked through the page table in tiles of 128 tokens (8 warps x 16), staged in shared memory by a 2..6-stage
 // cp.async pipeline (K and V rows, 16-byte chunks XOR-swizzled so that fragment reads are conflict-free):
 //   phase 1  thread = token: s[h] = q[h] . k  for the r heads (q pre-scaled, fp32, smem broadcast)
 //   softmax  online (running max / sum per head), warp-shuffle reductions, probabilities in smem
@@ -15,8 +15,9 @@
 
 namespace sagc {
 
-static constexpr int ATT_THREADS = 128;
-static constexpr int ATT_TILE = 64;          // tokens per pipeline stage
+static constexpr int ATT_WARPS = 8;          // each warp owns 16 tokens of a tile
+static constexpr int ATT_THREADS = ATT_WARPS * 32;
+static constexpr int ATT_TILE = ATT_WARPS * 16;   // tokens per pipeline stage
 static constexpr int ATT_MAXR = 8;
 static constexpr int ATT_MAXPG = 1104;       // page ids cached per split (17408 / 16 + slack)
 
@@ -43,7 +44,7 @@ template <int HD>
 struct AttSmem {
     static constexpr int ROWB = HD * 2;                       // unpadded rows, 16-byte chunks XOR-swizzled
     static constexpr int STAGE = 2 * ATT_TILE * ROWB;         // K rows then V rows
-    static constexpr int NSTAGE = HD >= 128 ? 3 : 6;           // K/V tiles in flight: NSTAGE - 1 (<= ~100 KB per CTA)
+    static constexpr int NSTAGE = HD >= 128 ? 2 : (HD >= 64 ? 3 : 6);           // K/V tiles in flight: NSTAGE - 1 (<= ~100 KB per CTA)
     static constexpr int BYTES = NSTAGE * STAGE;
 };
 
@@ -71,8 +72,8 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     constexpr int KB = HD / 32;                 // 32-wide d blocks
     constexpr int NT = HD / 8;                  // output n-tiles
     extern __shared__ __align__(128) unsigned char kv_s[];
-    __shared__ __align__(16) float o_w[4][ATT_MAXR][HD + 4];
-    __shared__ float m_w[4][ATT_MAXR], l_w[4][ATT_MAXR];
+    __shared__ __align__(16) float o_w[ATT_WARPS][ATT_MAXR][HD + 4];
+    __shared__ float m_w[ATT_WARPS][ATT_MAXR], l_w[ATT_WARPS][ATT_MAXR];
     __shared__ float m_s[ATT_MAXR], l_s[ATT_MAXR];
     __shared__ int last_s;
 
@@ -316,10 +317,12 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     }
     __syncthreads();
     if (tid < r) {
-        float mx = fmaxf(fmaxf(m_w[0][tid], m_w[1][tid]), fmaxf(m_w[2][tid], m_w[3][tid]));
+        float mx = m_w[0][tid];
+#pragma unroll
+        for (int w2 = 1; w2 < ATT_WARPS; ++w2) mx = fmaxf(mx, m_w[w2][tid]);
         float l = 0.f;
 #pragma unroll
-        for (int w2 = 0; w2 < 4; ++w2) l += (m_w[w2][tid] == -INFINITY) ? 0.f : __expf(m_w[w2][tid] - mx) * l_w[w2][tid];
+        for (int w2 = 0; w2 < ATT_WARPS; ++w2) l += (m_w[w2][tid] == -INFINITY) ? 0.f : __expf(m_w[w2][tid] - mx) * l_w[w2][tid];
         m_s[tid] = mx; l_s[tid] = l;
     }
     __syncthreads();
@@ -328,7 +331,7 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
         const float mx = m_s[h];
         float ov = 0.f;
 #pragma unroll
-        for (int w2 = 0; w2 < 4; ++w2)
+        for (int w2 = 0; w2 < ATT_WARPS; ++w2)
             ov += (m_w[w2][h] == -INFINITY) ? 0.f : __expf(m_w[w2][h] - mx) * o_w[w2][h][d];
         const int hq = kvh * r + h;
         if (nsp == 1) {
@@ -357,7 +360,7 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     // ---- merge: this CTA arrived last for (row, kvh) -----------------------------------------
     // warp w computes the normalised weight of every split for heads w, w+4 (lanes = splits) ...
     float* wgt = &o_w[0][0][0];                       // [r][nsp] (o_w is free again)
-    for (int h = warp; h < r; h += 4) {
+    for (int h = warp; h < r; h += ATT_WARPS) {
         const int hq = kvh * r + h;
         const float* ml = a.part_ml + ((size_t)row * a.Hq + hq) * nsp * 2;
         float mv[2], lv[2];
