@@ -132,13 +132,56 @@ struct TcCfg {
     static constexpr int TMEM_COLS = NA * NB <= 32 ? 32 : (NA * NB <= 64 ? 64 : (NA * NB <= 128 ? 128 : (NA * NB <= 256 ? 256 : 512)));
     static constexpr int TAIL = 1024;                                  // barriers, tmem slot, rstd, ssq scratch
     static constexpr int MAXSTAGES = (196 * 1024 / STAGE) > 8 ? 8 : (196 * 1024 / STAGE);
+    static constexpr bool PUSH_OK = NA * (NB / 2) * 128 * 4 <= 16 * 1024;   // keep the SwiGLU kernel at two CTAs per SM
+    static constexpr int RECV = PUSH_OK ? NA * (NB / 2) * 128 * 4 : 0;     // split-K partials pushed by the cluster peers
     static constexpr int EXCH = 32 * 128 * 4;                          // RoPE partner exchange (EPI_QKV)
     // the exchange buffer exists only in the EPI_QKV instantiation: 16 KB more would cost the SwiGLU kernel its
     // second CTA per SM (152 CTAs -> two waves)
-    static constexpr int smem_bytes(int stages, bool qkv) { return stages * STAGE + TAIL + 5 * MB * 4 + (qkv ? EXCH : 0) + 1024; }
+    static constexpr int smem_bytes(int stages, bool qkv) { return stages * STAGE + TAIL + 5 * MB * 4 + (qkv ? EXCH : 0) + RECV + 1024; }
 };
 
 __device__ __forceinline__ float silu_tc(float z) { return z / (1.f + __expf(-z)); }
+
+// TMEM -> (hi + lo) -> where the reduction will read it.  KS == 1: this CTA's shared memory.  KS > 1 and a
+// small partial tile (<= 16 KB): PUSHED straight into the shared memory of the cluster rank that owns the
+// column (remote stores are fire-and-forget, so the split-K exchange costs no load round trip; the tile is
+// <= 32 KB, well within DSMEM's ~20 B/clk).  Otherwise: the L2 scratch.
+template <int NB, int NA, int KS>
+__device__ __forceinline__ void tc_drain(const TcDev& a, cg::cluster_group& cluster, float* red, float* recv, uint32_t tmem_base,
+                                         int lg, int row, int rank, int cta_id, bool have_acc) {
+    constexpr int MB = NB / 2;
+    constexpr bool PUSH = (KS > 1) && TcCfg<NB, NA>::PUSH_OK;
+    float* rp[KS];
+    if (PUSH) {
+#pragma unroll
+        for (int d = 0; d < KS; ++d) rp[d] = cluster.map_shared_rank(recv, d);
+    }
+#pragma unroll
+    for (int na = 0; na < NA; ++na) {
+#pragma unroll
+        for (int c = 0; c < NB / 32; ++c) {
+            float v[32];
+            if (have_acc) {
+                tc_ld32(tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(na * NB + c * 32), v);
+            } else {
+#pragma unroll
+                for (int j = 0; j < 32; ++j) v[j] = 0.f;
+            }
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                const int m = c * 16 + j;
+                const float val = v[2 * j] + v[2 * j + 1];
+                if (KS == 1) {
+                    red[((size_t)na * MB + m) * 128 + row] = val;
+                } else if (PUSH) {
+                    rp[m % KS][(((size_t)rank * NA + na) * (MB / KS) + m / KS) * 128 + row] = val;
+                } else {
+                    __stcg(a.scratch + (size_t)cta_id * (NA * MB * 128) + ((size_t)na * MB + m) * 128 + row, val);
+                }
+            }
+        }
+    }
+}
 
 // Final epilogue of one CTA: rank r of a KS-way split finishes batch columns r, r+KS, ...  KS is a
 // compile-time constant so that EVERY load of a batch (all ranks' partial tiles from L2, or the local
@@ -146,13 +189,15 @@ __device__ __forceinline__ float silu_tc(float z) { return z / (1.f + __expf(-z)
 // batch of 64 / (NA*KS) columns, partials summed in rank order (deterministic).
 template <int NB, int EPI, int KS>
 __device__ __forceinline__ void tc_epilogue(const TcDev& a, const float* red, const float* rstd_s, float* ssq_s, float* exch,
-                                            int warp, int lane, int row0, int m0, int tile, int rank, int cta_id, int M, float nw) {
+                                            const float* recv, int warp, int lane, int row0, int m0, int tile, int rank, int cta_id,
+                                            int M, float nw) {
     constexpr int NA = (EPI == EPI_SWIGLU) ? 2 : 1;
     constexpr int MB = NB / 2;
     constexpr int MBATCH = (KS == 1) ? 16 / NA : 64 / (NA * KS);
     const int lg = warp & 3;
     const int row = lg * 32 + lane;
     const int n = row0 + row;
+    constexpr bool PUSH = (KS > 1) && TcCfg<NB, NA>::PUSH_OK;
     const float* base = (KS == 1) ? red : a.scratch + (size_t)(cta_id - rank) * (NA * MB * 128);
     for (int mb = rank; mb < MB; mb += KS * MBATCH) {
         if (m0 + mb >= M) break;
@@ -169,8 +214,12 @@ __device__ __forceinline__ void tc_epilogue(const TcDev& a, const float* red, co
             for (int j = 0; j < MBATCH; ++j)
 #pragma unroll
                 for (int na = 0; na < NA; ++na) {
-                    const float* src = base + (size_t)p * (NA * MB * 128) + ((size_t)na * MB + mc[j]) * 128 + row;
-                    v[p][j][na] = (KS == 1) ? *src : __ldcg(src);
+                    if (PUSH) {
+                        v[p][j][na] = recv[(((size_t)p * NA + na) * (MB / KS) + mc[j] / KS) * 128 + row];
+                    } else {
+                        const float* src = base + (size_t)p * (NA * MB * 128) + ((size_t)na * MB + mc[j]) * 128 + row;
+                        v[p][j][na] = (KS == 1) ? *src : __ldcg(src);
+                    }
                 }
         float outv[MBATCH], q2[MBATCH];
         uint32_t ohi[MBATCH], olo[MBATCH];
@@ -291,6 +340,7 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     float* rstd_s = reinterpret_cast<float*>(smem + S * C::STAGE + C::TAIL);
     float* ssq_s = rstd_s + MB;                                         // [4][MB]
     float* exch = ssq_s + 4 * MB;                                       // [32][128] (EPI_QKV)
+    float* recv = reinterpret_cast<float*>(smem + S * C::STAGE + C::TAIL + 5 * MB * 4 + (EPI == EPI_QKV ? C::EXCH : 0));   // pushed partials
     float* red = reinterpret_cast<float*>(smem);                        // [NA][MB][128], overlays the stages
 
     cg::cluster_group cluster = cg::this_cluster();
@@ -403,24 +453,32 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             tc_fence_after();
         }
         trace_mark_thread(8 * 4 + 1, 64);
+        if (C::PUSH_OK && KS > 1) {
+            switch (KS) {
+                case 2: tc_drain<NB, NA, 2>(a, cluster, red, recv, tmem_base, lg, row, rank, cta_id, nk > 0); break;
+                case 4: tc_drain<NB, NA, 4>(a, cluster, red, recv, tmem_base, lg, row, rank, cta_id, nk > 0); break;
+                default: tc_drain<NB, NA, 8>(a, cluster, red, recv, tmem_base, lg, row, rank, cta_id, nk > 0); break;
+            }
+        } else {
 #pragma unroll
-        for (int na = 0; na < NA; ++na) {
+            for (int na = 0; na < NA; ++na) {
 #pragma unroll
-            for (int c = 0; c < NB / 32; ++c) {
-                float v[32];
-                if (nk > 0) {
-                    tc_ld32(tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(na * NB + c * 32), v);
-                } else {
+                for (int c = 0; c < NB / 32; ++c) {
+                    float v[32];
+                    if (nk > 0) {
+                        tc_ld32(tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(na * NB + c * 32), v);
+                    } else {
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) v[j] = 0.f;
-                }
-                if (KS == 1) {
+                        for (int j = 0; j < 32; ++j) v[j] = 0.f;
+                    }
+                    if (KS == 1) {
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) red[((size_t)na * MB + c * 16 + j) * 128 + row] = v[2 * j] + v[2 * j + 1];
-                } else {      // split-K partials go through L2: far more bandwidth than DSMEM's ~20 B/clk per SM
-                    float* mine = a.scratch + (size_t)cta_id * (NA * MB * 128);
+                        for (int j = 0; j < 16; ++j) red[((size_t)na * MB + c * 16 + j) * 128 + row] = v[2 * j] + v[2 * j + 1];
+                    } else {      // large partial tiles go through the L2 scratch
+                        float* mine = a.scratch + (size_t)cta_id * (NA * MB * 128);
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) __stcg(mine + ((size_t)na * MB + c * 16 + j) * 128 + row, v[2 * j] + v[2 * j + 1]);
+                        for (int j = 0; j < 16; ++j) __stcg(mine + ((size_t)na * MB + c * 16 + j) * 128 + row, v[2 * j] + v[2 * j + 1]);
+                    }
                 }
             }
         }
@@ -437,10 +495,10 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     }
     if (warp >= 2) {
         switch (KS) {
-            case 1: tc_epilogue<NB, EPI, 1>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id, M_pre, nw_pre); break;
-            case 2: tc_epilogue<NB, EPI, 2>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id, M_pre, nw_pre); break;
-            case 4: tc_epilogue<NB, EPI, 4>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id, M_pre, nw_pre); break;
-            default: tc_epilogue<NB, EPI, 8>(a, red, rstd_s, ssq_s, exch, warp, lane, row0, m0, tile, rank, cta_id, M_pre, nw_pre); break;
+            case 1: tc_epilogue<NB, EPI, 1>(a, red, rstd_s, ssq_s, exch, recv, warp, lane, row0, m0, tile, rank, cta_id, M_pre, nw_pre); break;
+            case 2: tc_epilogue<NB, EPI, 2>(a, red, rstd_s, ssq_s, exch, recv, warp, lane, row0, m0, tile, rank, cta_id, M_pre, nw_pre); break;
+            case 4: tc_epilogue<NB, EPI, 4>(a, red, rstd_s, ssq_s, exch, recv, warp, lane, row0, m0, tile, rank, cta_id, M_pre, nw_pre); break;
+            default: tc_epilogue<NB, EPI, 8>(a, red, rstd_s, ssq_s, exch, recv, warp, lane, row0, m0, tile, rank, cta_id, M_pre, nw_pre); break;
         }
     }
     // no second cluster barrier: peers read this CTA's partials from the L2 scratch, never from its
