@@ -10,6 +10,8 @@
 // Split-K: split s covers tokens [s*cps, (s+1)*cps); partial (o, max, sum) go to scratch and the
 // last CTA to arrive for a (row, kv head) merges them with the log-sum-exp rule.
 // The same kernel serves prefill: every prompt position is a row with ctx = position + 1.
+#include <cooperative_groups.h>
+#include <cstdlib>
 #include "common.cuh"
 #include "kernels.cuh"
 
@@ -78,6 +80,10 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     __shared__ int last_s;
 
     __shared__ int pg_s[ATT_MAXPG];               // page ids of this split's blocks
+    // split merge inside a cluster (2..8 splits): every split pushes slice k of its un-normalised output and
+    // its (max, sum) pairs into the shared memory of cluster rank k, which combines and stores that slice
+    __shared__ float rv_o[ATT_MAXR * HD + 8];     // [split][slice]
+    __shared__ float rv_ml[8][ATT_MAXR][2];
     trace_mark(12);
     // Decode (a.prefetch): the live list, contexts, page table and every cached position but the
     // newest were written by EARLIER steps, so they may be read before the upstream kernel (this
@@ -86,7 +92,9 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     if (!a.prefetch) pdl_wait();
     const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
     const int row = blockIdx.x, kvh = blockIdx.y, split = blockIdx.z;
-    if (row >= M) { if (a.prefetch) pdl_wait(); pdl_launch(); return; }
+    if (row >= M) { if (a.prefetch) pdl_wait(); pdl_launch(); return; }      // uniform over the cluster (same row)
+    const bool cmerge = a.cluster_merge != 0;
+    if (cmerge) asm volatile("barrier.cluster.arrive.relaxed.aligned;\n" ::: "memory");   // "this CTA has started"; waited on before the pushes
     const int r = a.Hq / a.Hkv;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g = lane >> 2, q = lane & 3;
@@ -326,6 +334,10 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
         m_s[tid] = mx; l_s[tid] = l;
     }
     __syncthreads();
+    const int slice = (r * HD + nsp - 1) / nsp;
+    namespace cgn = cooperative_groups;
+    cgn::cluster_group cluster = cgn::this_cluster();
+    if (cmerge) asm volatile("barrier.cluster.wait.aligned;\n" ::: "memory");             // every peer is running
     for (int i = tid; i < r * HD; i += ATT_THREADS) {
         const int h = i / HD, d = i % HD;
         const float mx = m_s[h];
@@ -336,11 +348,41 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
         const int hq = kvh * r + h;
         if (nsp == 1) {
             store_out(a, row, hq * HD + d, ov / l_s[h]);
+        } else if (cmerge) {
+            const int owner = i / slice;
+            cluster.map_shared_rank(rv_o, owner)[split * slice + (i - owner * slice)] = ov;
         } else {
             a.part_o[(((size_t)row * a.Hq + hq) * nsp + split) * HD + d] = ov;
         }
     }
     if (nsp == 1) { trace_mark(3 * 4 + 2); return; }
+    if (cmerge) {
+        if (tid < r * nsp) {
+            const int h = tid / nsp, dst = tid % nsp;
+            float* ml = &cluster.map_shared_rank(rv_ml, dst)[split][h][0];
+            ml[0] = m_s[h];
+            ml[1] = l_s[h];
+        }
+        cluster.sync();                           // release the pushes / acquire the peers'
+        const int total = r * HD;
+        for (int e = tid; e < slice; e += ATT_THREADS) {
+            const int i = split * slice + e;
+            if (i >= total) break;
+            const int h = i / HD, d = i % HD;
+            float mx = -INFINITY;
+            for (int s2 = 0; s2 < nsp; ++s2) mx = fmaxf(mx, rv_ml[s2][h][0]);
+            float num = 0.f, den = 0.f;
+            for (int s2 = 0; s2 < nsp; ++s2) {
+                const float l2 = rv_ml[s2][h][1];
+                const float f = (l2 > 0.f) ? __expf(rv_ml[s2][h][0] - mx) : 0.f;
+                den += f * l2;
+                num += f * rv_o[s2 * slice + e];
+            }
+            store_out(a, row, (kvh * r + h) * HD + d, num / den);
+        }
+        trace_mark(3 * 4 + 2);
+        return;
+    }
     if (tid < r) {
         const int hq = kvh * r + tid;
         float* ml = a.part_ml + (((size_t)row * a.Hq + hq) * nsp + split) * 2;
@@ -403,6 +445,20 @@ static int launch_att(const AttnArgs& a, cudaStream_t st) {
         attr_set = true;
     }
     dim3 grid(a.m_max, a.Hkv, a.n_splits);
+    static const bool use_cluster = [] { const char* e = getenv("SAGC_ATT_CLUSTER"); return e ? atoi(e) != 0 : true; }();
+    if (use_cluster && a.n_splits > 1 && a.n_splits <= 8) {
+        AttnArgs ac = a;
+        ac.cluster_merge = 1;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = grid; cfg.blockDim = dim3(ATT_THREADS); cfg.dynamicSmemBytes = AttSmem<HD>::BYTES; cfg.stream = st;
+        cudaLaunchAttribute at[2];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = 1; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = a.n_splits;
+        at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[1].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = g_pdl_all ? 2 : 1;
+        return cudaLaunchKernelEx(&cfg, k_attention<HD>, ac) == cudaSuccess ? 1 : -1;
+    }
     launch_pdl(k_attention<HD>, grid, dim3(ATT_THREADS), AttSmem<HD>::BYTES, st, g_pdl_all, a);
     return 1;
 }

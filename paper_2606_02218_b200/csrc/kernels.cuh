@@ -70,6 +70,7 @@ struct AttnArgs {
     // position happen inside this kernel (no separate RoPE kernel).  head_dim >= 64.
     int fuse_rope; const float* rope_cs; const int* row_pos; bf16_t* kv_layer_w;
     int prefetch;           // 1 in decode: cached positions older than the newest one predate the upstream kernel
+    int cluster_merge;      // set by the launcher: the n_splits CTAs of a (row, kv head) form a cluster and merge through DSMEM
 };
 int launch_attention(const AttnArgs& a, cudaStream_t st);
 

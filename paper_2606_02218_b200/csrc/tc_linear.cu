@@ -127,12 +127,14 @@ struct TcCfg {
     static constexpr int B_BYTES = NB * 128;
     static constexpr int STAGE = NA * A_BYTES + B_BYTES;
     // ~100 KB of stages per CTA so that two CTAs share an SM (one's epilogue overlaps the other's loads)
-    static constexpr int STAGES = (100 * 1024 / STAGE) < 2 ? 2 : ((100 * 1024 / STAGE) > 6 ? 6 : (100 * 1024 / STAGE));
+    // SwiGLU at UMMA N = 32 (36 KB stages): three stages and no receive buffer still fit two CTAs per SM (111 KB each)
+    static constexpr bool GU32 = (NA == 2 && NB == 32);
+    static constexpr int STAGES = GU32 ? 3 : ((100 * 1024 / STAGE) < 2 ? 2 : ((100 * 1024 / STAGE) > 6 ? 6 : (100 * 1024 / STAGE)));
     static constexpr int MB = NB / 2;
     static constexpr int TMEM_COLS = NA * NB <= 32 ? 32 : (NA * NB <= 64 ? 64 : (NA * NB <= 128 ? 128 : (NA * NB <= 256 ? 256 : 512)));
     static constexpr int TAIL = 1024;                                  // barriers, tmem slot, rstd, ssq scratch
     static constexpr int MAXSTAGES = (196 * 1024 / STAGE) > 8 ? 8 : (196 * 1024 / STAGE);
-    static constexpr bool PUSH_OK = NA * (NB / 2) * 128 * 4 <= 16 * 1024;   // keep the SwiGLU kernel at two CTAs per SM
+    static constexpr bool PUSH_OK = !GU32 && NA * (NB / 2) * 128 * 4 <= 16 * 1024;   // keep the SwiGLU kernel at two CTAs per SM
     static constexpr int RECV = PUSH_OK ? NA * (NB / 2) * 128 * 4 : 0;     // split-K partials pushed by the cluster peers
     static constexpr int EXCH = 32 * 128 * 4;                          // RoPE partner exchange (EPI_QKV)
     // the exchange buffer exists only in the EPI_QKV instantiation: 16 KB more would cost the SwiGLU kernel its
