@@ -464,6 +464,8 @@ static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
     if (want > m->max_splits) want = m->max_splits;
     int s = 1;
     while (s * 2 <= want) s *= 2;
+    static const int smax = env_int("SAGC_ATT_MAXSPLIT", 8);      // <= 8 splits merge inside a cluster (attention.cu)
+    if (s > smax) s = smax;
     return s;
 }
 
