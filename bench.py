@@ -157,8 +157,23 @@ def kernel_roofline(B, torch, mc, peak):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / n
     nbytes = N * K * 2 + M * K * 4 + M * N * 4
-    return {"kernel": "k_linear_tc<128,STORE> (LM head, 64 live rows; + k_split_rows)", "bytes": nbytes, "ms": ms,
-            "achieved_gbs": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak}
+    out = {"kernel": "k_linear_tc<128,STORE> (LM head, 64 live rows; + k_split_rows)", "bytes": nbytes, "ms": ms,
+           "achieved_gbs": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak}
+    # the launch the decode step actually uses at <= 64 live rows: LM head + Gumbel sampler fused (logits never stored)
+    sids = torch.arange(M, dtype=torch.int32, device="cuda")
+    for _ in range(3):
+        B.debug_lm_sample(W, x, sids, 5, seed=7)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(n):
+        B.debug_lm_sample(W, x, sids, 5, seed=7)
+    e1.record()
+    torch.cuda.synchronize()
+    ms2 = e0.elapsed_time(e1) / n
+    nb2 = N * K * 2 + M * K * 4
+    out["fused"] = {"kernel": "k_lmhead_sample<128> (persistent LM head + Philox Gumbel arg-max, 64 live rows; + k_split_rows, k_pick_candidates)",
+                    "bytes": nb2, "ms": ms2, "achieved_gbs": nb2 / ms2 / 1e6, "frac": nb2 / ms2 / 1e6 / peak}
+    return out
 
 
 def main():

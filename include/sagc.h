@@ -180,6 +180,16 @@ int sagc_debug_philox(uint64_t seed, int32_t sid, int32_t t, int32_t v0, int32_t
  *   W dev bf16 [N][K], x dev float [M][K], y dev float [M][N]. */
 int sagc_debug_linear(const void* W, const float* x, float* y, int32_t M, int32_t N, int32_t K,
                       int32_t path, void* stream);
+/* Fused LM head + sampler of a decode step (steps a11 + a12: logits never stored), as a unit:
+ *   tokens[m] = argmax_v( (x[m] . W[v]) / temperature + Gumbel(Philox(seed; sids[m], t, v)) )   (mode 1)
+ *             = argmax_v(  x[m] . W[v] ), lowest v on exact ties                               (mode 0)
+ *   W dev bf16 [V][K], x dev float [M][K] (1 <= M <= 64), sids dev int32 [M], out_tokens dev int32 [M],
+ *   out_logits dev float [M][V] or NULL (optional dump of the logits the epilogue saw).  V % 128 == 0,
+ *   K % 64 == 0.  Synchronises the stream when (mode, temperature, seed, t) change (parameter upload);
+ *   returns SAGC_EINVAL on bad shapes. */
+int sagc_debug_lm_sample(const void* W, const float* x, int32_t M, int32_t V, int32_t K, int32_t mode, float temperature,
+                         uint64_t seed, int32_t t, const int32_t* sids, int32_t* out_tokens, float* out_logits,
+                         void* stream);
 /* One paged GQA decode-attention call over a caller-built cache (unit test of step a7):
  *   q dev float [M][Hq][hd]; kv dev bf16 pool laid out as the model lays it out for ONE layer:
  *   [n_pages][2][Hkv][page_tokens][hd]; page_table dev int32 [M][max_blocks]; ctx dev int32 [M];

@@ -27,7 +27,7 @@ EXPORTS = [
     "sagc_model_create", "sagc_model_destroy", "sagc_rollout_group", "sagc_rollout_group_host",
     "sagc_group_advantage", "sagc_length_stats", "sagc_debug_page_table", "sagc_debug_free_stack",
     "sagc_debug_alloc_log", "sagc_debug_retire_log", "sagc_debug_peak_pages", "sagc_debug_philox",
-    "sagc_debug_linear", "sagc_debug_attention", "sagc_last_error", "sagc_version",
+    "sagc_debug_linear", "sagc_debug_lm_sample", "sagc_debug_attention", "sagc_last_error", "sagc_version",
 ]
 
 
@@ -93,6 +93,8 @@ def lib():
         L.sagc_debug_philox.argtypes = [C.c_uint64, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         L.sagc_debug_linear.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
                                         C.c_void_p]
+        L.sagc_debug_lm_sample.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_float,
+                                           C.c_uint64, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.sagc_debug_attention.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32,
                                            C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         _lib = L
@@ -302,6 +304,19 @@ def debug_linear(W_bits: torch.Tensor, x: torch.Tensor, path: int = PATH_GEMM) -
     y = torch.empty((M, N), dtype=torch.float32, device=x.device)
     _check(lib().sagc_debug_linear(W_bits.data_ptr(), x.data_ptr(), y.data_ptr(), M, N, K, path, _stream()))
     return y
+
+
+def debug_lm_sample(W_bits: torch.Tensor, x: torch.Tensor, sids: torch.Tensor, t: int, mode: int = MODE_GUMBEL,
+                    temperature: float = 1.0, seed: int = 0, want_logits: bool = False):
+    """Fused LM head + sampler: W_bits int16 [V][K], x float32 [M][K], sids int32 [M] -> tokens int32 [M] (, logits [M][V])."""
+    _require_cuda()
+    V, K = W_bits.shape
+    M = x.shape[0]
+    tok = torch.empty((M,), dtype=torch.int32, device=x.device)
+    lg = torch.empty((M, V), dtype=torch.float32, device=x.device) if want_logits else None
+    _check(lib().sagc_debug_lm_sample(W_bits.data_ptr(), x.data_ptr(), M, V, K, mode, temperature, seed, t, sids.data_ptr(),
+                                      tok.data_ptr(), lg.data_ptr() if want_logits else None, _stream()))
+    return (tok, lg) if want_logits else tok
 
 
 def debug_attention(q: torch.Tensor, kv_bits: torch.Tensor, page_table: torch.Tensor, ctx: torch.Tensor, Hq: int,

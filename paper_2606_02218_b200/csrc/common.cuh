@@ -54,6 +54,23 @@ __device__ __forceinline__ void prefetch_l2(const void* p) {
     asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p));
 }
 
+// Gumbel draw of the sampler from one Philox word (step a12):  u = ((x >> 9) + 0.5) * 2^-23,  g = -log(-log u).
+// Two MUFU.LG2 instead of two full-range logf: the inner log is taken as the series of -log(1 - e) with
+// e = 1 - u formed EXACTLY when u is within 2^-6 of 1 (that is where the largest draws -- the likely winners
+// of the arg-max -- live and where lg2 alone loses all relative accuracy); elsewhere |log u| > 0.0157 and the
+// 2^-22 absolute error of lg2 is < 2e-5 relative.  |g - exact| < ~3e-5 over the whole range, far below the
+// 1e-2 top-2 margin of the token rule.  Used by BOTH sampler paths (k_sample and the
+// fused LM head) so that they pick identical tokens.
+__device__ __forceinline__ float gumbel_from_u32(uint32_t x) {
+    const float k = (float)(x >> 9);                               // 0 .. 2^23 - 1, exact
+    const float u = (k + 0.5f) * 1.1920928955078125e-07f;          // exact in fp32
+    const float e = (8388607.5f - k) * 1.1920928955078125e-07f;    // 1 - u, exact
+    const float y_near1 = fmaf(e * e, fmaf(e, 0.33333334f, 0.5f), e);
+    const float y_far = -__logf(u);
+    const float y = (e < 0.015625f) ? y_near1 : y_far;
+    return -__logf(y);
+}
+
 // ---- programmatic dependent launch (griddepcontrol) ---------------------------------
 // pdl_wait(): block until the upstream grid's memory is visible (no-op without the PDL attr).
 // pdl_launch(): allow the downstream grid to start its prologue.

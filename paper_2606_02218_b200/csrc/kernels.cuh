@@ -116,7 +116,8 @@ int launch_prefill_alloc(const PageState& ps, const RolloutDev& rd, cudaStream_t
 // End of step t (retire / free / compact) + start of step t+1 (page alloc, pos/ctx/tok).
 // `sampled` holds the sampler's token for each live slot; first_step: slots are sids (t = 1).
 int launch_advance(const PageState& ps, const RolloutDev& rd, const float* part_score, const int* part_tok,
-                   int structure_only, cudaStream_t st);
+                   int structure_only, cudaStream_t st, int n_parts = 32 /* SMP_CHUNKS */, int part_sc = 1,
+                   int part_si = 32);      // candidate c of slot i at [c * part_sc + i * part_si]
 // Prefill helpers: row_sid/row_pos/row_ctx/tok for every prompt token, and the copy of a partial
 // last prompt block into the first private page of completions g >= 1.
 int launch_prefill_rows(const int* prompt_tokens, const int* prompt_offsets_dev, int n_prompts, int G,
@@ -153,6 +154,22 @@ struct TcLinearArgs {
     bool pdl;
 };
 int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st);
+// Fused final norm + LM head + sampler (persistent tcgen05 kernel, <= 64 live rows).  Steps a11 + a12.
+static constexpr int LM_MAX_PARTS = 160;                     // candidates per row = CTAs of the fused kernel
+struct LmSampleArgs {
+    const TcMap* a;             // lm_head map (box 64 x 128)
+    const TcMap* b;             // pre-split activation map for the chosen N
+    int K, V;
+    const int* m_dev; int m_max;
+    const float* ssq_in; int ssq_in_tiles; int ssq_ld; float eps; int k_norm;
+    const int* row_sid; const int* step_dev; const uint32_t* params;
+    float* part_score; int* part_tok; int part_ld;           // [lm_sample_grid(V)][part_ld]
+    float* Y; int ldy;          // optional logits dump (null in the product path)
+    bool pdl;
+};
+int lm_sample_grid(int V);
+int launch_lmhead_sample(const LmSampleArgs& t, cudaStream_t st);
+int launch_pick_candidates(const float* part_score, const int* part_tok, int n_parts, int ld, int M, int* out_tok, cudaStream_t st);
 int launch_embed_split(const bf16_t* embed, const int* tok, const int* m_dev, int m_max, int d, float* x,
                        const bf16_t* norm_w, bf16_t* xs, float* ssq, int ssq_ld, int ssq_tiles, cudaStream_t st);
 int launch_split_rows(const float* x, int K, const int* m_dev, int m_max, bf16_t* xs, cudaStream_t st);

@@ -120,7 +120,8 @@ int launch_prefill_alloc(const PageState& ps, const RolloutDev& rd, cudaStream_t
 
 // End of step t + start of step t+1.  One CTA, thread i = live slot i.
 __global__ void __launch_bounds__(PG_THREADS) k_advance(PageState ps, RolloutDev rd, const float* part_score,
-                                                        const int* part_tok, int structure_only) {
+                                                        const int* part_tok, int structure_only, int n_parts,
+                                                        int part_sc, int part_si) {
     __shared__ int warp_s[33];
     __shared__ int grp_live[1024], grp_ret[1024], grp_last[1024];
     trace_mark(28); pdl_wait(); trace_mark(29);
@@ -131,6 +132,25 @@ __global__ void __launch_bounds__(PG_THREADS) k_advance(PageState ps, RolloutDev
     if (*ps.err) return;
     int n_free = *ps.n_free;
     for (int k = i; k < rd.n_prompts; k += PG_THREADS) { grp_live[k] = 0; grp_ret[k] = 0; grp_last[k] = -1; }
+    // fused LM head + sampler: one candidate per CTA ([c][64] layout, <= 64 live rows).  All 1024 threads fetch them
+    // in ONE round trip (thread = row i % 64, candidate subset i / 64), then slot i takes the best of 16 from shared memory.
+    __shared__ float cand_s[16][64];
+    __shared__ int cand_t[16][64];
+    const bool wide = n_parts > 32 && part_si == 1 && !structure_only && !rd.forced_tok;
+    if (wide) {
+        const int r = i & 63, p = i >> 6;
+        float b = -INFINITY;
+        int ix = 0x7fffffff;
+        if (r < n_live) {
+#pragma unroll 10
+            for (int c = p; c < n_parts; c += 16) {
+                const float s2 = part_score[(size_t)c * part_sc + r];
+                const int t2 = part_tok[(size_t)c * part_sc + r];
+                if (s2 > b || (s2 == b && t2 < ix)) { b = s2; ix = t2; }
+            }
+        }
+        cand_s[p][r] = b; cand_t[p][r] = ix;
+    }
     __syncthreads();
 
     // ---- append token, decide retirement ---------------------------------------------
@@ -142,12 +162,25 @@ __global__ void __launch_bounds__(PG_THREADS) k_advance(PageState ps, RolloutDev
         if (rd.forced_tok) tokv = rd.forced_tok[(size_t)sid * rd.max_new + (t - 1)];
         else if (!structure_only) {
             // best of the sampler's per-slice candidates, ascending slices: lowest index wins ties
-            float bs = part_score[i * SMP_CHUNKS];
-            tokv = part_tok[i * SMP_CHUNKS];
-            for (int c = 1; c < SMP_CHUNKS; ++c) {
-                const float s2 = part_score[i * SMP_CHUNKS + c];
-                const int t2 = part_tok[i * SMP_CHUNKS + c];
-                if (s2 > bs || (s2 == bs && t2 < tokv)) { bs = s2; tokv = t2; }
+            // candidate c of slot i sits at [c * part_sc + i * part_si] (k_sample: slices; fused LM head: CTAs)
+            float bs;
+            if (wide) {
+                bs = cand_s[0][i]; tokv = cand_t[0][i];
+#pragma unroll
+                for (int c = 1; c < 16; ++c) {
+                    const float s2 = cand_s[c][i];
+                    const int t2 = cand_t[c][i];
+                    if (s2 > bs || (s2 == bs && t2 < tokv)) { bs = s2; tokv = t2; }
+                }
+            } else {
+                bs = part_score[(size_t)i * part_si];
+                tokv = part_tok[(size_t)i * part_si];
+#pragma unroll 8
+                for (int c = 1; c < n_parts; ++c) {
+                    const float s2 = part_score[(size_t)c * part_sc + (size_t)i * part_si];
+                    const int t2 = part_tok[(size_t)c * part_sc + (size_t)i * part_si];
+                    if (s2 > bs || (s2 == bs && t2 < tokv)) { bs = s2; tokv = t2; }
+                }
             }
         }
         rd.out_tokens[(size_t)sid * rd.max_new + (t - 1)] = tokv;
@@ -231,8 +264,9 @@ __global__ void __launch_bounds__(PG_THREADS) k_advance(PageState ps, RolloutDev
     }
 }
 int launch_advance(const PageState& ps, const RolloutDev& rd, const float* part_score, const int* part_tok,
-                   int structure_only, cudaStream_t st) {
-    launch_pdl(k_advance, dim3(1), dim3(PG_THREADS), 0, st, g_pdl_all, ps, rd, part_score, part_tok, structure_only);
+                   int structure_only, cudaStream_t st, int n_parts, int part_sc, int part_si) {
+    launch_pdl(k_advance, dim3(1), dim3(PG_THREADS), 0, st, g_pdl_all, ps, rd, part_score, part_tok, structure_only, n_parts,
+               part_sc, part_si);
     return 1;
 }
 

@@ -82,6 +82,8 @@ struct sagc_model {
     // scratch activations
     float *x, *qkv, *att, *act, *logits, *xlast, *part_o, *part_ml;
     float* part_score;
+    float* lm_score; int* lm_tok;              // fused LM head + sampler: [lm_sample_grid][64] candidates
+    int lm_fused;                              // SAGC_LM_FUSED (default 1): decode steps with <= 64 live rows and no logits dump
     int *counters, *sampled, *row_sid, *row_pos, *row_ctx, *row_tok, *last_idx, *prompt_len_d, *offs_d;
     int row_cap;
     // per-call device buffers (grown on demand)
@@ -182,6 +184,7 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     sagc::g_pdl_all = m->use_pdl && env_int("SAGC_PDL_ALL", 1) != 0;
     m->gemv_max = env_int("SAGC_GEMV_MAX", 0);
     m->skip_mask = env_int("SAGC_SKIP", 0);
+    m->lm_fused = env_int("SAGC_LM_FUSED", 1);
     m->tc_min = env_int("SAGC_TC_MIN", 1);   // measured: the tcgen05 path beats the register-HMMA tail kernels at every batch size
     m->tok_buf = m->len_buf = m->forced_len_d = m->dump_list_d = m->prompt_tok_d = nullptr;
     m->tok_cap = m->forced_cap = m->dump_cap = m->prompt_cap = 0;
@@ -230,6 +233,7 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     cudaMemset(m->counters, 0, R * c.n_kv_heads * sizeof(int));
     DA(m->sampled, (size_t)c.max_seqs * SMP_CHUNKS); DA(m->part_score, (size_t)c.max_seqs * SMP_CHUNKS); DA(m->last_idx, c.max_seqs); DA(m->prompt_len_d, c.max_seqs);
     DA(m->offs_d, c.max_seqs + 1);
+    DA(m->lm_score, (size_t)LM_MAX_PARTS * 64); DA(m->lm_tok, (size_t)LM_MAX_PARTS * 64);
     DA(m->sample_params_d, 4);
     m->last_nseq = 0; m->last_max_blocks = m->max_blocks;
     {
@@ -477,6 +481,20 @@ static int enqueue_decode_step(sagc_model* m, const RolloutDev& rd, int m_bucket
     RowSet rs = {m->ps.live, m->ps.pos, m->ps.ctx, m->ps.tok, m->ps.n_live, m_bucket};
     int n = enqueue_layers(m, rs, n_splits, kind, st);
     if (n < 0) return -1;
+    const sagc_model_config& c = m->cfg;
+    if (m->lm_fused && kind == LIN_TC && m_bucket <= 64 && n_dump == 0 && (c.vocab % 128) == 0 && !(m->skip_mask & (2 | 16))) {
+        // a11 + a12 in one persistent kernel: the logits never reach HBM
+        LmSampleArgs f = {};
+        f.a = &m->wmaps[(size_t)c.n_layers * 7]; f.b = &m->amaps[0][tc_nb_index(m_bucket)]; f.K = c.d_model; f.V = c.vocab;
+        f.m_dev = m->ps.n_live; f.m_max = m_bucket; f.ssq_in = m->ssq; f.ssq_in_tiles = m->d_tiles; f.ssq_ld = m->ssq_ld;
+        f.eps = c.rms_eps; f.k_norm = c.d_model; f.row_sid = m->ps.live; f.step_dev = m->ps.step; f.params = m->sample_params_d;
+        f.part_score = m->lm_score; f.part_tok = m->lm_tok; f.part_ld = 64; f.Y = nullptr; f.ldy = c.vocab; f.pdl = m->use_pdl;
+        int r = launch_lmhead_sample(f, st);
+        if (r < 0) return -1;
+        n += r;
+        n += launch_advance(m->ps, rd, m->lm_score, m->lm_tok, 0, st, lm_sample_grid(c.vocab), 64, 1);
+        return n;
+    }
     int r = enqueue_lm_head(m, m->x, m->ps.n_live, m_bucket, kind, st);
     if (r < 0) return -1;
     n += r;
@@ -924,6 +942,53 @@ extern "C" int sagc_debug_linear(const void* W, const float* x, float* y, int32_
     a.W[0] = reinterpret_cast<const bf16_t*>(W); a.rows[0] = N; a.X = x; a.Y = y; a.ldy = N; a.K = K; a.N = N;
     a.m_dev = nullptr; a.m_max = M; a.epi = EPI_STORE; a.kind = (path == SAGC_PATH_GEMV) ? LIN_GEMV : LIN_MMA; a.pdl = false;
     if (launch_linear(a, st) < 0) return set_err(SAGC_ECUDA, "launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    CU(cudaGetLastError());
+    return SAGC_OK;
+}
+extern "C" int sagc_debug_lm_sample(const void* W, const float* x, int32_t M, int32_t V, int32_t K, int32_t mode, float temperature,
+                                    uint64_t seed, int32_t t, const int32_t* sids, int32_t* out_tokens, float* out_logits,
+                                    void* stream) {
+    if (!W || !x || !sids || !out_tokens || M < 1 || M > 64 || V % 128 || K % 64 || temperature <= 0.f)
+        return set_err(SAGC_EINVAL, "need 1 <= M <= 64, V %% 128 == 0, K %% 64 == 0, temperature > 0");
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const int nbi = tc_nb_index(M), NB = 32 << nbi;
+    static bf16_t* xs = nullptr;                // debug entry: grow-only buffers, kept for the process lifetime
+    static size_t xs_cap = 0;
+    static float* ps = nullptr; static int* pt = nullptr; static uint32_t* prm = nullptr; static int* step = nullptr;
+    const size_t rows = (size_t)NB;
+    if (rows * K > xs_cap) {
+        CU(cudaDeviceSynchronize());
+        if (xs) cudaFree(xs);
+        xs_cap = rows * K;
+        CU(cudaMalloc(&xs, xs_cap * sizeof(bf16_t)));
+        CU(cudaMemset(xs, 0, xs_cap * sizeof(bf16_t)));
+    }
+    if (!ps) {
+        CU(cudaMalloc(&ps, (size_t)LM_MAX_PARTS * 64 * sizeof(float)));
+        CU(cudaMalloc(&pt, (size_t)LM_MAX_PARTS * 64 * sizeof(int)));
+        CU(cudaMalloc(&prm, 4 * sizeof(uint32_t)));
+        CU(cudaMalloc(&step, sizeof(int)));
+    }
+    uint32_t hp[4];
+    hp[0] = (uint32_t)mode; memcpy(&hp[1], &temperature, 4); hp[2] = (uint32_t)(seed & 0xffffffffu); hp[3] = (uint32_t)(seed >> 32);
+    static uint32_t last_hp[4] = {~0u, 0u, 0u, 0u};
+    static int last_t = -1;
+    if (memcmp(hp, last_hp, sizeof(hp)) != 0 || t != last_t) {      // repeated calls (timing loops) skip the upload
+        CU(cudaMemcpyAsync(prm, hp, sizeof(hp), cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(step, &t, sizeof(int), cudaMemcpyHostToDevice, st));
+        CU(cudaStreamSynchronize(st));          // hp / t live on this frame
+        memcpy(last_hp, hp, sizeof(hp)); last_t = t;
+    }
+    launch_split_rows(x, K, nullptr, M, xs, st);
+    TcMap ma, mb;
+    if (tc_make_map(&ma, W, V, K, 128) != 0 || tc_make_map(&mb, xs, (long long)rows, K, NB) != 0)
+        return set_err(SAGC_ECUDA, "cuTensorMapEncodeTiled failed");
+    LmSampleArgs f = {};
+    f.a = &ma; f.b = &mb; f.K = K; f.V = V; f.m_dev = nullptr; f.m_max = M; f.ssq_in = nullptr; f.k_norm = K;
+    f.row_sid = sids; f.step_dev = step; f.params = prm; f.part_score = ps; f.part_tok = pt; f.part_ld = 64;
+    f.Y = out_logits; f.ldy = V; f.pdl = false;
+    if (launch_lmhead_sample(f, st) < 0) return set_err(SAGC_ECUDA, "fused LM head: %s", cudaGetErrorString(cudaGetLastError()));
+    launch_pick_candidates(ps, pt, lm_sample_grid(V), 64, M, out_tokens, st);
     CU(cudaGetLastError());
     return SAGC_OK;
 }

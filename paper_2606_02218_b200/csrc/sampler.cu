@@ -1,7 +1,7 @@
 // sampler.cu -- greedy / Philox-keyed Gumbel-max sampler (steps a3, a12).
 //   Philox4x32-10, key = (seed lo, seed hi), counter = (v >> 2, t, sid, 0); word v & 3 is the
-//   draw for vocab id v.  u = ((x >> 9) + 0.5) * 2^-23;  g = -log(-log u);
-//   token = argmax_v(logit_v / T + g_v), lowest v on exact ties (reading C2).
+//   draw for vocab id v.  u = ((x >> 9) + 0.5) * 2^-23;  g = -log(-log u) (gumbel_from_u32, common.cuh);
+//   token = argmax_v(logit_v * (1 / T) + g_v), lowest v on exact ties (reading C2).
 #include "common.cuh"
 #include "kernels.cuh"
 
@@ -18,11 +18,6 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
         k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
     }
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
-}
-
-__device__ __forceinline__ float gumbel_from_u32(uint32_t x) {
-    const float u = ((float)(x >> 9) + 0.5f) * 1.1920928955078125e-07f;   // 2^-23, exact in fp32
-    return -logf(-logf(u));
 }
 
 __global__ void k_philox_debug(uint32_t k0, uint32_t k1, int sid, int t, int v0, int n, uint32_t* out) {
@@ -60,7 +55,7 @@ __global__ void __launch_bounds__(SMP_THREADS) k_sample(SampleArgs a) {
     const float* lg = a.logits + (size_t)(row / a.row_div) * a.V;
     const int sid = a.row_sid[row];
     const int mode = (int)a.params[0];
-    const float temperature = __uint_as_float(a.params[1]);
+    const float inv_t = 1.f / __uint_as_float(a.params[1]);
     const uint32_t k0 = a.params[2], k1 = a.params[3];
     const int t = *a.step_dev;
     float bs = -INFINITY;
@@ -82,7 +77,7 @@ __global__ void __launch_bounds__(SMP_THREADS) k_sample(SampleArgs a) {
             uint32_t w[4];
             philox4x32_10((uint32_t)b, (uint32_t)t, (uint32_t)sid, 0u, k0, k1, w);
 #pragma unroll
-            for (int e = 0; e < 4; ++e) s[e] = s[e] / temperature + gumbel_from_u32(w[e]);
+            for (int e = 0; e < 4; ++e) s[e] = fmaf(s[e], inv_t, gumbel_from_u32(w[e]));
         }
 #pragma unroll
         for (int e = 0; e < 4; ++e)

@@ -646,4 +646,326 @@ int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
     return e == cudaSuccess ? 1 : -1;
 }
 
+
+// =============================================================================================
+// k_lmhead_sample -- final norm + LM head + sampler in ONE persistent kernel (steps a11 + a12; SURVEY
+// 8(a): "fuse with a12 so logits [M][V] fp32 never hit HBM").  One CTA per SM walks the vocabulary
+// tiles  blockIdx.x, blockIdx.x + gridDim.x, ...: the TMA ring runs ahead across tile boundaries and the
+// accumulator is double-buffered in TMEM, so the epilogue of tile j (TMEM -> logit -> Philox Gumbel
+// perturbation -> running arg-max in registers) overlaps the weight stream of tile j+1.  Each CTA
+// writes ONE (score, token) candidate per batch row; k_advance takes the best of the gridDim.x
+// candidates (ties: lowest token id, the comparator is order-independent).
+// Philox block (v >> 2, t, sid) is shared by the four lanes that hold vocab ids 4b..4b+3: lane q of the
+// quad computes the block of batch row m0 + q and the words are exchanged by shuffles, so no block is
+// computed twice.  Accumulator slot x of a quad therefore holds batch row m0 + (x ^ q) (undone at the end).
+// =============================================================================================
+struct LmDev {
+    int n_kb, tiles, V;
+    const int* m_dev; int m_max;
+    const float* ssq_in; int ssq_in_tiles, ssq_ld; float eps; int k_norm;
+    int stages;
+    const int* row_sid; const int* step_dev; const uint32_t* params;
+    float* part_score; int* part_tok; int part_ld;      // [gridDim.x][part_ld]
+    float* Y; int ldy;                                  // optional logits dump (parity / debugging), may be null
+};
+
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void lm_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t k0, uint32_t k1, uint32_t (&out)[4]) {
+    uint32_t c3 = 0u;
+#pragma unroll
+    for (int i = 0; i < 10; ++i) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+template <typename T>
+__device__ __forceinline__ T sel4(T a0, T a1, T a2, T a3, int i) {
+    const T lo = (i & 1) ? a1 : a0, hi = (i & 1) ? a3 : a2;
+    return (i & 2) ? hi : lo;
+}
+
+static constexpr int LM_EPI_THREADS = 256;                    // 8 epilogue warps
+static constexpr int LM_THREADS = 64 + LM_EPI_THREADS;       // + TMA producer warp + MMA issuer warp
+
+template <int NB>
+__global__ void __launch_bounds__(LM_THREADS, 1)
+k_lmhead_sample(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, LmDev a) {
+    constexpr int MB = NB / 2;
+    constexpr int A_BYTES = 128 * 128, STAGE = A_BYTES + NB * 128;
+    const int S = a.stages;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem + S * STAGE);
+    uint64_t* empty = full + S;
+    uint64_t* tfull = empty + S;           // [2] accumulator slot complete
+    uint64_t* tempty = tfull + 2;          // [2] accumulator slot drained by the eight epilogue warps
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
+    float* rstd_s = reinterpret_cast<float*>(smem + S * STAGE + 512);
+    int* sid_s = reinterpret_cast<int*>(rstd_s + MB);
+    float* red_sc = reinterpret_cast<float*>(smem);            // [MB][128] final reduction, overlays the ring
+    int* red_ix = reinterpret_cast<int*>(red_sc + MB * 128);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_my = (a.tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;    // tiles of this CTA
+    const int total = n_my * a.n_kb;
+
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], LM_EPI_THREADS / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(tmem_slot)), "n"(2 * NB));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp == 0) {
+        // ===== TMA producer: one flat iteration space over (tile, k block) =====
+        if (lane == 0) {
+            tma_prefetch_desc(&tmA);
+            tma_prefetch_desc(&tmB);
+            const int pre = min(S, total);
+            for (int i = 0; i < pre; ++i) {       // weights never depend on the upstream kernel
+                const int tile = (int)blockIdx.x + (i / a.n_kb) * (int)gridDim.x, kb = i % a.n_kb;
+                mbar_expect_tx(&full[i], STAGE);
+                tma_load_2d(smem + i * STAGE, &tmA, &full[i], kb * TC_BK, tile * 128);
+            }
+            pdl_wait();
+            for (int i = 0; i < pre; ++i) tma_load_2d(smem + i * STAGE + A_BYTES, &tmB, &full[i], (i % a.n_kb) * TC_BK, 0);
+            for (int i = pre; i < total; ++i) {
+                const int s = i % S;
+                const int tile = (int)blockIdx.x + (i / a.n_kb) * (int)gridDim.x, kb = i % a.n_kb;
+                mbar_wait(&empty[s], ((i / S) - 1) & 1);
+                mbar_expect_tx(&full[s], STAGE);
+                tma_load_2d(smem + s * STAGE, &tmA, &full[s], kb * TC_BK, tile * 128);
+                tma_load_2d(smem + s * STAGE + A_BYTES, &tmB, &full[s], kb * TC_BK, 0);
+            }
+        }
+        pdl_launch();
+    } else if (warp == 1) {
+        // ===== MMA issuer =====
+        pdl_launch();
+        const uint32_t idesc = umma_idesc(NB);
+        int i = 0;
+        for (int j = 0; j < n_my; ++j) {
+            const int slot = j & 1, use = j >> 1;
+            if (use > 0) { mbar_wait(&tempty[slot], (use - 1) & 1); tc_fence_after(); }
+            for (int kb = 0; kb < a.n_kb; ++kb, ++i) {
+                const int s = i % S;
+                mbar_wait(&full[s], (i / S) & 1);
+                tc_fence_after();
+                if (lane == 0) {
+                    const uint32_t sa = smem_u32(smem + s * STAGE);
+                    const uint64_t adesc = umma_desc_sw128(sa), bdesc = umma_desc_sw128(sa + A_BYTES);
+#pragma unroll
+                    for (int k = 0; k < TC_BK / 16; ++k)
+                        tc_mma(tmem_base + slot * NB, adesc + 2 * k, bdesc + 2 * k, idesc, (kb > 0 || k > 0) ? 1u : 0u);
+                    tc_commit(&empty[s]);
+                    if (kb == a.n_kb - 1) tc_commit(&tfull[slot]);
+                }
+                __syncwarp();
+            }
+        }
+    } else {
+        // ===== epilogue warps: logits -> perturbed scores -> running arg-max =====
+        // Eight warps: TMEM lane group lg = warp % 4 is served by two warps (h = 0, 1) that split the batch
+        // columns, so every SM sub-partition holds two independent instruction streams (the Philox / logf
+        // chains are latency-bound in a single warp).
+        constexpr int NCH = NB / 32;                  // 32-column TMEM chunks = 16 batch rows each
+        constexpr int SLOTS = MB / 2;                 // batch rows per warp
+        const int lg = warp & 3, row = lg * 32 + lane, q = lane & 3, h = (warp - 2) >> 2;
+        pdl_wait();
+        pdl_launch();
+        const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
+        const int et = (warp - 2) * 32 + lane;        // 0..255
+        for (int m = et; m < MB; m += LM_EPI_THREADS) {
+            float t = 0.f;
+            if (a.ssq_in != nullptr)
+                for (int i = 0; i < a.ssq_in_tiles; ++i) t += a.ssq_in[(size_t)i * a.ssq_ld + m];
+            rstd_s[m] = (a.ssq_in != nullptr) ? rsqrtf(t / (float)a.k_norm + a.eps) : 1.f;
+            sid_s[m] = (m < M) ? a.row_sid[m] : 0;
+        }
+        const int mode = (int)a.params[0];
+        const float inv_t = 1.f / __uint_as_float(a.params[1]);
+        const uint32_t k0 = a.params[2], k1 = a.params[3];
+        const uint32_t tstep = (uint32_t)*a.step_dev;
+        asm volatile("bar.sync 1, 256;\n" ::: "memory");
+        float bs[SLOTS];
+        int bi[SLOTS];
+#pragma unroll
+        for (int m = 0; m < SLOTS; ++m) { bs[m] = -INFINITY; bi[m] = 0x7fffffff; }
+        for (int j = 0; j < n_my; ++j) {
+            const int slot = j & 1;
+            const int v = ((int)blockIdx.x + j * (int)gridDim.x) * 128 + row;      // this thread's vocab id in tile j
+            mbar_wait(&tfull[slot], (j >> 1) & 1);
+            tc_fence_after();
+#pragma unroll
+            for (int ci = 0; ci < (NCH == 1 ? 1 : NCH / 2); ++ci) {
+                const int c = (NCH == 1) ? 0 : 2 * ci + h;                 // this warp's chunk
+                const int g_lo = (NCH == 1) ? 2 * h : 0;                   // and its quads of 4 batch rows
+                constexpr int NG = (NCH == 1) ? 2 : 4;
+                const bool live = (c * 16 + 4 * g_lo) < M;                 // warp-uniform
+                float acc[32];
+                if (live) tc_ld32(tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)(slot * NB + c * 32), acc);
+                if (ci == (NCH == 1 ? 1 : NCH / 2) - 1) {                  // slot drained by this warp
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&tempty[slot]);
+                }
+                if (!live) continue;
+                float L[4 * NG];
+#pragma unroll
+                for (int i = 0; i < 4 * NG; ++i) {
+                    float sum = acc[2 * i] + acc[2 * i + 1];
+                    if constexpr (NCH == 1) {         // the warp's columns start at 8 * h (h is runtime: select, static indices)
+                        const float hi = acc[2 * (i + 8)] + acc[2 * (i + 8) + 1];
+                        sum = h ? hi : sum;
+                    }
+                    L[i] = sum * rstd_s[c * 16 + 4 * g_lo + i];
+                }
+                if (a.Y != nullptr) {
+#pragma unroll
+                    for (int i = 0; i < 4 * NG; ++i) {
+                        const int mrow = c * 16 + 4 * g_lo + i;
+                        if (mrow < M) a.Y[(size_t)mrow * a.ldy + v] = L[i];
+                    }
+                }
+                uint32_t W[NG][4];
+                if (mode == 1) {
+#pragma unroll
+                    for (int g = 0; g < NG; ++g)      // independent Philox chains: no early exit between them
+                        lm_philox((uint32_t)v >> 2, tstep, (uint32_t)sid_s[c * 16 + 4 * (g_lo + g) + q], k0, k1, W[g]);
+                }
+#pragma unroll
+                for (int g = 0; g < NG; ++g) {
+#pragma unroll
+                    for (int x = 0; x < 4; ++x) {
+                        const int mm = q ^ x;                                  // batch row (quad base) + mm sits in slot x
+                        float sc = sel4(L[4 * g], L[4 * g + 1], L[4 * g + 2], L[4 * g + 3], mm);
+                        if (mode == 1) {
+                            // lane q' = q ^ x computed the block of row base + q'; this lane needs its word q
+                            const uint32_t send = sel4(W[g][0], W[g][1], W[g][2], W[g][3], mm);
+                            const uint32_t w = (x == 0) ? send : __shfl_xor_sync(0xffffffffu, send, x);
+                            sc = fmaf(sc, inv_t, gumbel_from_u32(w));
+                        }
+                        const int sl = ci * 16 + 4 * g + x;
+                        if (sc > bs[sl]) { bs[sl] = sc; bi[sl] = v; }          // tiles ascend: strict > keeps the lowest id
+                    }
+                }
+            }
+        }
+        // ---- best over the 128 vocabulary lanes of this CTA, one candidate per batch row ----
+        // (the last tfull wait implies every MMA has finished reading the ring: safe to overlay)
+        asm volatile("bar.sync 1, 256;\n" ::: "memory");
+#pragma unroll
+        for (int sl = 0; sl < SLOTS; ++sl) {
+            const int ci = sl >> 4, r4 = sl & 15;
+            const int base = (NCH == 1) ? 8 * h + (r4 & ~3) : (2 * ci + h) * 16 + (r4 & ~3);
+            const int mt = base + ((r4 & 3) ^ q);
+            red_sc[mt * 128 + row] = bs[sl];
+            red_ix[mt * 128 + row] = bi[sl];
+        }
+        asm volatile("bar.sync 1, 256;\n" ::: "memory");
+        if (et < MB && et < M) {
+            float b = -INFINITY;
+            int ix = 0x7fffffff;
+#pragma unroll 8
+            for (int i = 0; i < 128; ++i) {
+                const int r = (i + et) & 127;
+                const float s2 = red_sc[et * 128 + r];
+                const int i2 = red_ix[et * 128 + r];
+                if (s2 > b || (s2 == b && i2 < ix)) { b = s2; ix = i2; }
+            }
+            a.part_score[(size_t)blockIdx.x * a.part_ld + et] = b;
+            a.part_tok[(size_t)blockIdx.x * a.part_ld + et] = ix;
+        }
+        tc_fence_before();
+    }
+    __syncthreads();
+    if (warp == 2) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "n"(2 * NB));
+    }
+}
+
+template <int NB>
+static cudaError_t launch_lm_inst(const LmSampleArgs& t, LmDev d, int grid, cudaStream_t st) {
+    constexpr int STAGE = 128 * 128 + NB * 128;
+    int stages = (196 * 1024) / STAGE;
+    if (stages > 10) stages = 10;
+    d.stages = stages;
+    const int smem = stages * STAGE + 512 + (NB / 2) * 8 + 1024;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(k_lmhead_sample<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(LM_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = t.pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, k_lmhead_sample<NB>, *reinterpret_cast<const CUtensorMap*>(t.a),
+                              *reinterpret_cast<const CUtensorMap*>(t.b), d);
+}
+
+// best of the per-CTA candidates (debug entry; in a rollout k_advance does this)
+__global__ void k_pick_candidates(const float* part_score, const int* part_tok, int n_parts, int ld, int M, int* out_tok) {
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= M) return;
+    float b = part_score[m];
+    int ix = part_tok[m];
+    for (int c = 1; c < n_parts; ++c) {
+        const float s2 = part_score[(size_t)c * ld + m];
+        const int i2 = part_tok[(size_t)c * ld + m];
+        if (s2 > b || (s2 == b && i2 < ix)) { b = s2; ix = i2; }
+    }
+    out_tok[m] = ix;
+}
+int launch_pick_candidates(const float* part_score, const int* part_tok, int n_parts, int ld, int M, int* out_tok, cudaStream_t st) {
+    k_pick_candidates<<<1, 64, 0, st>>>(part_score, part_tok, n_parts, ld, M, out_tok);
+    return 1;
+}
+
+int lm_sample_grid(int V) {
+    const char* e = getenv("SAGC_LM_CTAS");          // read per call (graph build time): tests force several tiles per CTA
+    const int g = (e && atoi(e) > 0) ? atoi(e) : 148;
+    const int tiles = V / 128;
+    return tiles < g ? tiles : (g > LM_MAX_PARTS ? LM_MAX_PARTS : g);
+}
+
+int launch_lmhead_sample(const LmSampleArgs& t, cudaStream_t st) {
+    if (t.m_max <= 0) return 0;
+    if (t.m_max > 64 || (t.V % 128) != 0 || (t.K % TC_BK) != 0) return -1;
+    LmDev d;
+    d.n_kb = t.K / TC_BK; d.tiles = t.V / 128; d.V = t.V; d.m_dev = t.m_dev; d.m_max = t.m_max; d.ssq_in = t.ssq_in;
+    d.ssq_in_tiles = t.ssq_in_tiles; d.ssq_ld = t.ssq_ld; d.eps = t.eps; d.k_norm = t.k_norm; d.stages = 0;
+    d.row_sid = t.row_sid; d.step_dev = t.step_dev; d.params = t.params; d.part_score = t.part_score; d.part_tok = t.part_tok;
+    d.part_ld = t.part_ld; d.Y = t.Y; d.ldy = t.ldy;
+    const int grid = lm_sample_grid(t.V);
+    cudaError_t e;
+    switch (tc_nb_index(t.m_max)) {
+        case 0: e = launch_lm_inst<32>(t, d, grid, st); break;
+        case 1: e = launch_lm_inst<64>(t, d, grid, st); break;
+        default: e = launch_lm_inst<128>(t, d, grid, st); break;
+    }
+    return e == cudaSuccess ? 1 : -1;
+}
+
 }  // namespace sagc

@@ -117,6 +117,38 @@ def test_linear_vs_fp64(B, N, K, M, path):
     assert np.max(np.abs(y - ref)) < 3e-5 * max(1.0, scale), np.max(np.abs(y - ref))
 
 
+# ---------------------------------------------------------------------------- a11 + a12 fused
+@pytest.mark.parametrize("M,V,K,ctas", [(1, 1024, 128, 148), (5, 4096, 256, 3), (16, 4096, 896, 7), (17, 8192, 256, 148),
+                                        (40, 4096, 256, 5), (64, 151936, 896, 148)])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_fused_lm_head_sampler_vs_oracle(B, monkeypatch, M, V, K, ctas, mode):
+    """Persistent tcgen05 LM head with the sampler in its epilogue: dumped logits vs fp64, tokens vs the oracle's
+    Philox-Gumbel arg-max on fp64 logits (token equal, or the oracle's top-2 margin of the perturbed scores < 1e-2)."""
+    monkeypatch.setenv("SAGC_LM_CTAS", str(ctas))
+    rng = np.random.default_rng(V + 7 * K + M + mode)
+    Wb = wl.f32_to_bf16_bits((0.02 * rng.standard_normal((V, K))).astype(np.float32))
+    x = rng.standard_normal((M, K)).astype(np.float32)
+    sids = rng.permutation(1000)[:M].astype(np.int32)
+    t, seed, T = 37, (0xABCD << 32) | 99, 0.7
+    ref = x.astype(np.float64) @ wl.bf16_bits_to_f32(Wb).astype(np.float64).T
+    tok, lg = B.debug_lm_sample(_dev(Wb.view(np.int16)), _dev(x), _dev(sids), t, mode=mode, temperature=T, seed=seed,
+                                want_logits=True)
+    tok2 = B.debug_lm_sample(_dev(Wb.view(np.int16)), _dev(x), _dev(sids), t, mode=mode, temperature=T, seed=seed)
+    tok, lg = tok.cpu().numpy(), lg.cpu().numpy()
+    assert np.array_equal(tok, tok2.cpu().numpy())          # the logits dump does not change the pick
+    assert np.max(np.abs(lg - ref)) < 3e-5 * max(1.0, np.sqrt(K) * 0.02)
+    n_eq = 0
+    for m in range(M):
+        sc = oph.perturbed_scores(ref[m].astype(np.float32), mode, T, seed, int(sids[m]), t)
+        best = int(np.argmax(sc))
+        n_eq += int(tok[m] == best)
+        assert tok[m] == best or oph.top2_margin(sc) < 1e-2, (m, tok[m], best)
+        # the kernel's own logits must reproduce its pick exactly (same arithmetic as the unfused sampler)
+        sc_k = oph.perturbed_scores(lg[m], mode, T, seed, int(sids[m]), t)
+        assert abs(float(sc_k[tok[m]]) - float(sc_k.max())) <= 1e-4
+    assert n_eq >= M - max(1, M // 16)
+
+
 # ---------------------------------------------------------------------------- a7
 @pytest.mark.parametrize("Hq,Hkv,hd,page", [(4, 4, 32, 16), (14, 2, 64, 64), (28, 4, 128, 64), (8, 1, 128, 32)])
 def test_paged_attention_vs_fp64(B, Hq, Hkv, hd, page):

@@ -329,3 +329,29 @@ def test_no_graph_flag_gives_identical_tokens(B):
     for a, b in zip(outs[0], outs[1]):
         assert np.array_equal(a, b)
     m.close()
+
+
+@pytest.mark.parametrize("G,mode,ctas", [(3, "gumbel", 5), (20, "gumbel", 3), (20, "greedy", 148), (9, "gumbel", 148)])
+def test_fused_lm_head_sampler_gives_identical_tokens(B, monkeypatch, G, mode, ctas):
+    """a11 + a12 fused (persistent tcgen05 LM head with the Gumbel arg-max in its epilogue, logits never stored) against the
+    unfused LM head -> k_sample path: the logit arithmetic and the Philox keys are the same, so tokens must be identical.
+    SAGC_LM_CTAS forces several vocabulary tiles per CTA (TMEM double buffer, ring wrap-around, ragged tile counts)."""
+    w = wl.tiny_variant(1, model_n_q_heads=4, model_n_kv_heads=2, model_head_dim=64, model_d_model=256,
+                        model_d_ff=512, model_n_layers=2, model_vocab=8192, model_page_tokens=16)
+    weights = wl.make_weights(w.model, 5)
+    prompts, offs = wl.make_prompts(w, n_prompts=2, prompt_len=20)
+    rng = np.random.default_rng(G)
+    fl = rng.integers(1, 25, size=2 * G).astype(np.int32)
+    fl[0] = 24
+    outs = []
+    for fused in ("1", "0"):
+        monkeypatch.setenv("SAGC_LM_FUSED", fused)
+        monkeypatch.setenv("SAGC_LM_CTAS", str(ctas))
+        m = B.Model(w.model, weights, 200, 2 * G, 20 + 24)
+        out = m.rollout_group(prompts, offs, G, mode=B.MODE_GUMBEL if mode == "gumbel" else B.MODE_GREEDY, temperature=0.8,
+                              seed=23, max_new_tokens=24, forced_lengths=fl, flags=B.FLAG_LOG)
+        outs.append((out.tokens.cpu().numpy(), out.lengths.cpu().numpy(), m.debug_page_table()))
+        m.close()
+    for a, b in zip(outs[0], outs[1]):
+        assert np.array_equal(a, b)
+    assert (outs[0][0] >= 0).sum() == int(fl.sum())
