@@ -664,6 +664,7 @@ struct LmDev {
     const int* m_dev; int m_max;
     const float* ssq_in; int ssq_in_tiles, ssq_ld; float eps; int k_norm;
     int stages;
+    int bres;                                           // activations (all k blocks) stay resident in shared memory
     const int* row_sid; const int* step_dev; const uint32_t* params;
     float* part_score; int* part_tok; int part_ld;      // [gridDim.x][part_ld]
     float* Y; int ldy;                                  // optional logits dump (parity / debugging), may be null
@@ -698,15 +699,22 @@ __global__ void __launch_bounds__(LM_THREADS, 1)
 k_lmhead_sample(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, LmDev a) {
     constexpr int MB = NB / 2;
     constexpr int A_BYTES = 128 * 128, STAGE = A_BYTES + NB * 128;
+    constexpr int B_BYTES = NB * 128;
     const int S = a.stages;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem + S * STAGE);
+    // bres: [n_kb activation tiles, loaded once][ring of weight-only stages]; else: ring of (weight + activation) stages.
+    // The activation tile of a k block is the same for every vocabulary tile: keeping it resident removes it from the
+    // per-stage L2 -> SM traffic (a quarter of it at UMMA N = 32, a third at N = 64).
+    const int stage_sz = a.bres ? A_BYTES : STAGE;
+    uint8_t* ring = smem + (a.bres ? a.n_kb * B_BYTES : 0);
+    uint64_t* full = reinterpret_cast<uint64_t*>(ring + S * stage_sz);
     uint64_t* empty = full + S;
     uint64_t* tfull = empty + S;           // [2] accumulator slot complete
     uint64_t* tempty = tfull + 2;          // [2] accumulator slot drained by the eight epilogue warps
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
-    float* rstd_s = reinterpret_cast<float*>(smem + S * STAGE + 512);
+    uint64_t* bfull = tempty + 2;          // resident activations landed (bres)
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bfull + 1);
+    float* rstd_s = reinterpret_cast<float*>(ring + S * stage_sz + 512);
     int* sid_s = reinterpret_cast<int*>(rstd_s + MB);
     float* red_sc = reinterpret_cast<float*>(smem);            // [MB][128] final reduction, overlays the ring
     int* red_ix = reinterpret_cast<int*>(red_sc + MB * 128);
@@ -718,6 +726,7 @@ k_lmhead_sample(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
         for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], LM_EPI_THREADS / 32); }
+        mbar_init(bfull, 1);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     if (warp == 2) {
@@ -737,18 +746,23 @@ k_lmhead_sample(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             const int pre = min(S, total);
             for (int i = 0; i < pre; ++i) {       // weights never depend on the upstream kernel
                 const int tile = (int)blockIdx.x + (i / a.n_kb) * (int)gridDim.x, kb = i % a.n_kb;
-                mbar_expect_tx(&full[i], STAGE);
-                tma_load_2d(smem + i * STAGE, &tmA, &full[i], kb * TC_BK, tile * 128);
+                mbar_expect_tx(&full[i], stage_sz);
+                tma_load_2d(ring + i * stage_sz, &tmA, &full[i], kb * TC_BK, tile * 128);
             }
             pdl_wait();
-            for (int i = 0; i < pre; ++i) tma_load_2d(smem + i * STAGE + A_BYTES, &tmB, &full[i], (i % a.n_kb) * TC_BK, 0);
+            if (a.bres) {
+                mbar_expect_tx(bfull, a.n_kb * B_BYTES);
+                for (int kb = 0; kb < a.n_kb; ++kb) tma_load_2d(smem + kb * B_BYTES, &tmB, bfull, kb * TC_BK, 0);
+            } else {
+                for (int i = 0; i < pre; ++i) tma_load_2d(ring + i * STAGE + A_BYTES, &tmB, &full[i], (i % a.n_kb) * TC_BK, 0);
+            }
             for (int i = pre; i < total; ++i) {
                 const int s = i % S;
                 const int tile = (int)blockIdx.x + (i / a.n_kb) * (int)gridDim.x, kb = i % a.n_kb;
                 mbar_wait(&empty[s], ((i / S) - 1) & 1);
-                mbar_expect_tx(&full[s], STAGE);
-                tma_load_2d(smem + s * STAGE, &tmA, &full[s], kb * TC_BK, tile * 128);
-                tma_load_2d(smem + s * STAGE + A_BYTES, &tmB, &full[s], kb * TC_BK, 0);
+                mbar_expect_tx(&full[s], stage_sz);
+                tma_load_2d(ring + s * stage_sz, &tmA, &full[s], kb * TC_BK, tile * 128);
+                if (!a.bres) tma_load_2d(ring + s * STAGE + A_BYTES, &tmB, &full[s], kb * TC_BK, 0);
             }
         }
         pdl_launch();
@@ -757,6 +771,7 @@ k_lmhead_sample(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         pdl_launch();
         const uint32_t idesc = umma_idesc(NB);
         int i = 0;
+        if (a.bres) { mbar_wait(bfull, 0); tc_fence_after(); }
         for (int j = 0; j < n_my; ++j) {
             const int slot = j & 1, use = j >> 1;
             if (use > 0) { mbar_wait(&tempty[slot], (use - 1) & 1); tc_fence_after(); }
@@ -765,8 +780,9 @@ k_lmhead_sample(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                 mbar_wait(&full[s], (i / S) & 1);
                 tc_fence_after();
                 if (lane == 0) {
-                    const uint32_t sa = smem_u32(smem + s * STAGE);
-                    const uint64_t adesc = umma_desc_sw128(sa), bdesc = umma_desc_sw128(sa + A_BYTES);
+                    const uint32_t sa = smem_u32(ring + s * stage_sz);
+                    const uint64_t adesc = umma_desc_sw128(sa);
+                    const uint64_t bdesc = umma_desc_sw128(a.bres ? smem_u32(smem + kb * B_BYTES) : sa + A_BYTES);
 #pragma unroll
                     for (int k = 0; k < TC_BK / 16; ++k)
                         tc_mma(tmem_base + slot * NB, adesc + 2 * k, bdesc + 2 * k, idesc, (kb > 0 || k > 0) ? 1u : 0u);
@@ -900,14 +916,20 @@ k_lmhead_sample(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
 
 template <int NB>
 static cudaError_t launch_lm_inst(const LmSampleArgs& t, LmDev d, int grid, cudaStream_t st) {
-    constexpr int STAGE = 128 * 128 + NB * 128;
-    int stages = (196 * 1024) / STAGE;
+    constexpr int A_BYTES = 128 * 128, B_BYTES = NB * 128, STAGE = A_BYTES + B_BYTES;
+    // SAGC_LM_BRES: 0 = activation tile re-fetched with every stage, 1 = resident at UMMA N = 32, 2 = also at N = 64
+    // (only when at least four weight stages still fit beside it)
+    static const int bres_knob = [] { const char* e = getenv("SAGC_LM_BRES"); return e ? atoi(e) : 0; }();
+    const int b_all = d.n_kb * B_BYTES;
+    const bool want = (bres_knob >= 1 && NB == 32) || (bres_knob >= 2 && NB == 64);
+    d.bres = (want && b_all + 4 * A_BYTES <= 196 * 1024) ? 1 : 0;
+    int stages = d.bres ? (196 * 1024 - b_all) / A_BYTES : (196 * 1024) / STAGE;
     if (stages > 10) stages = 10;
     d.stages = stages;
-    const int smem = stages * STAGE + 512 + (NB / 2) * 8 + 1024;
+    const int smem = (d.bres ? b_all + stages * A_BYTES : stages * STAGE) + 512 + (NB / 2) * 8 + 1024;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_lmhead_sample<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(k_lmhead_sample<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
