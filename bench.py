@@ -172,7 +172,9 @@ def kernel_roofline(B, torch, mc, peak):
     ms2 = e0.elapsed_time(e1) / n
     nb2 = N * K * 2 + M * K * 4
     out["fused"] = {"kernel": "k_lmhead_sample<128> (persistent LM head + Philox Gumbel arg-max, 64 live rows; + k_split_rows, k_pick_candidates)",
-                    "bytes": nb2, "ms": ms2, "achieved_gbs": nb2 / ms2 / 1e6, "frac": nb2 / ms2 / 1e6 / peak}
+                    "bytes": nb2, "ms": ms2, "achieved_gbs": nb2 / ms2 / 1e6, "frac": nb2 / ms2 / 1e6 / peak,
+                    # dram__bytes_read.sum of this kernel at this shape, one launch (profiles/r01_ncu_top_kernels.md)
+                    "traffic": 272578048 if (N, K) == (151936, 896) else None}
     return out
 
 
