@@ -138,6 +138,15 @@ def allreduce_max(values, device, world):
     return [float(x) for x in t]
 
 
+SHAPE_NAMES = {1: "tiny", 2: "0.5B", 3: "1.5B", 4: "7B", 5: "7B"}
+
+
+def decode_weight_bytes(mc):
+    """bf16 weight bytes one decode step reads (W)."""
+    q, kv = mc.n_q_heads * mc.head_dim, mc.n_kv_heads * mc.head_dim
+    return 2 * (mc.n_layers * (mc.d_model * q + 2 * mc.d_model * kv + q * mc.d_model + 3 * mc.d_model * mc.d_ff) + mc.vocab * mc.d_model)
+
+
 def kernel_roofline(B, torch, mc, peak):
     """Time the largest single launch of a decode step alone (LM head, M = 64): CUDA events on the
     launching stream, weights (272 MB) larger than L2 so every iteration streams from HBM."""
@@ -285,10 +294,11 @@ def main():
     line = {"metric": METRIC, "value": world * acc["tokens"] / ms * 1e3, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-            "config": {"workload": f"configs[{args.cfg - 1}]: 0.5B-shaped decoder, {w.n_prompts} prompts x {w.prompt_len} tokens x G={w.G}, "
-                                   f"forced lengths lognormal(median 1024, sigma 0.8) cap {max_new}, Gumbel T=1 Philox",
+            "config": {"workload": f"configs[{args.cfg - 1}]: {SHAPE_NAMES.get(args.cfg, '?')}-shaped decoder, {w.n_prompts} prompts x {w.prompt_len} tokens x G={w.G}, "
+                                   f"forced lengths {w.length_kind}({w.length_scale:g}, {w.length_shape:g}) cap {max_new}, "
+                                   f"{'Gumbel T=%g Philox' % w.temperature if w.sampling == 'gumbel' else 'greedy'}",
                        "tokens_per_step": acc["tokens"] // args.steps,
-                       "precision": "bf16 weights and KV cache, activations carried as hi+lo bf16 pairs (~16 mantissa bits), fp32 accumulate", "l2": "weights 0.99 GB per decode step > 126 MB L2",
+                       "precision": "bf16 weights and KV cache, activations carried as hi+lo bf16 pairs (~16 mantissa bits), fp32 accumulate", "l2": "weights %.2f GB per decode step > 126 MB L2" % (decode_weight_bytes(mc) / 1e9),
                        "replicas": world},
             "clocks": clocks, "gpu_launches": acc["launches"],
             "e2e": {"value": world * e2e_tok / e2e_ms * 1e3, "unit": UNIT, "h2d_bytes_per_step": int(prompts.nbytes + fl.nbytes),
