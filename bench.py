@@ -223,6 +223,10 @@ def main():
     page = mc.page_tokens
     nseq = w.n_prompts * w.G
     n_pages = w.n_prompts * (w.prompt_len // page + w.G * ((max_new + page - 1) // page + 1)) + 8
+    if n_pages * page * 2 * mc.n_layers * mc.n_kv_heads * mc.head_dim * 2 > 100e9:
+        # worst case (every completion at the cap) does not fit: size the pool for the forced lengths actually drawn
+        # (an upper bound that needs no retirement: every sequence's own blocks + the shared prefix blocks)
+        n_pages = int(np.sum((fl + page - 1) // page + 2)) + w.n_prompts * (w.prompt_len // page + 1) + 8
     model = B.Model(mc, weights, n_pages, nseq, w.prompt_len + max_new, device=f"cuda:{local}")
     mode = B.MODE_GUMBEL if w.sampling == "gumbel" else B.MODE_GREEDY
     adv_mode = B.ADV_DAPO if w.adv_mode == "DAPO" else B.ADV_GRPO
