@@ -174,6 +174,11 @@ int sagc_debug_alloc_log(sagc_model* m, int32_t* out, int32_t capacity, int32_t*
 int sagc_debug_retire_log(sagc_model* m, int32_t* out, int32_t capacity, int32_t* n);
 /* Peak number of pages in use during the last rollout. */
 int sagc_debug_peak_pages(sagc_model* m, int32_t* peak);
+/* In-kernel timeline of the persistent decode-step kernel (only when the handle was created with the environment
+ * variable SAGC_STEP_TRACE=1; otherwise *n = 0): copies the (tag, nanosecond) pairs recorded so far to out HOST
+ * uint64 [capacity][2] and arms the recording of decode step `record_step` (1-based step index) of the next rollout.
+ * tag = cta << 40 | role << 32 | event << 16 | phase. */
+int sagc_debug_step_trace(sagc_model* m, int64_t record_step, uint64_t* out, int32_t capacity, int32_t* n);
 /* Philox4x32-10 draws of the sampler for vocab ids v0..v0+n-1 of (seed, sid, t): out dev uint32 [n]. */
 int sagc_debug_philox(uint64_t seed, int32_t sid, int32_t t, int32_t v0, int32_t n, uint32_t* out, void* stream);
 /* y[M][N] = x[M][K] . W[N][K]^T through the projection kernels (path = SAGC_PATH_GEMV | _GEMM).
@@ -193,10 +198,14 @@ int sagc_debug_lm_sample(const void* W, const float* x, int32_t M, int32_t V, in
 /* One paged GQA decode-attention call over a caller-built cache (unit test of step a7):
  *   q dev float [M][Hq][hd]; kv dev bf16 pool laid out as the model lays it out for ONE layer:
  *   [n_pages][2][Hkv][page_tokens][hd]; page_table dev int32 [M][max_blocks]; ctx dev int32 [M];
- *   out dev float [M][Hq][hd]. */
+ *   out dev float [M][Hq][hd].  n_splits (1..64) = K-splits per (row, kv head).
+ *   variant 0: the standalone kernel (one CTA per unit; 2..8 splits merge inside a cluster through DSMEM,
+ *              more through the L2 scratch);  variant 1: the units as the persistent decode-step kernel runs
+ *              them (one CTA per SM looping over units, last-arriver merge; head_dim 64 / 128 only).
+ *   Synchronises the stream.  SAGC_EINVAL on bad shapes. */
 int sagc_debug_attention(const float* q, const void* kv, const int32_t* page_table, const int32_t* ctx,
                          int32_t M, int32_t Hq, int32_t Hkv, int32_t hd, int32_t page_tokens,
-                         int32_t max_blocks, float* out, void* stream);
+                         int32_t max_blocks, int32_t n_splits, int32_t variant, float* out, void* stream);
 
 const char* sagc_last_error(void);
 const char* sagc_version(void);

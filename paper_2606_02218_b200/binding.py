@@ -27,7 +27,7 @@ EXPORTS = [
     "sagc_model_create", "sagc_model_destroy", "sagc_rollout_group", "sagc_rollout_group_host",
     "sagc_group_advantage", "sagc_length_stats", "sagc_debug_page_table", "sagc_debug_free_stack",
     "sagc_debug_alloc_log", "sagc_debug_retire_log", "sagc_debug_peak_pages", "sagc_debug_philox",
-    "sagc_debug_linear", "sagc_debug_lm_sample", "sagc_debug_attention", "sagc_last_error", "sagc_version",
+    "sagc_debug_linear", "sagc_debug_lm_sample", "sagc_debug_attention", "sagc_debug_step_trace", "sagc_last_error", "sagc_version",
 ]
 
 
@@ -96,7 +96,9 @@ def lib():
         L.sagc_debug_lm_sample.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_float,
                                            C.c_uint64, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.sagc_debug_attention.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32,
-                                           C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
+                                           C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p,
+                                           C.c_void_p]
+        L.sagc_debug_step_trace.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_int32, C.POINTER(C.c_int32)]
         _lib = L
     return _lib
 
@@ -258,6 +260,13 @@ class Model:
     def debug_retire_log(self) -> np.ndarray:
         return self._log(lib().sagc_debug_retire_log, 2, self.max_seqs)
 
+    def debug_step_trace(self, record_step: int) -> np.ndarray:
+        """(tag, ns) pairs recorded by the persistent decode-step kernel so far; arms step `record_step` of the next rollout."""
+        out = np.zeros((16000, 2), dtype=np.uint64)
+        n = C.c_int32()
+        _check(lib().sagc_debug_step_trace(self._h, int(record_step), out.ctypes.data, 16000, C.byref(n)))
+        return out[: n.value].copy()
+
     def debug_peak_pages(self) -> int:
         p = C.c_int32()
         _check(lib().sagc_debug_peak_pages(self._h, C.byref(p)))
@@ -320,11 +329,13 @@ def debug_lm_sample(W_bits: torch.Tensor, x: torch.Tensor, sids: torch.Tensor, t
 
 
 def debug_attention(q: torch.Tensor, kv_bits: torch.Tensor, page_table: torch.Tensor, ctx: torch.Tensor, Hq: int,
-                    Hkv: int, hd: int, page_tokens: int) -> torch.Tensor:
-    """q float32 [M][Hq][hd]; kv_bits int16 [n_pages][2][Hkv][page][hd]; page_table int32 [M][max_blocks]."""
+                    Hkv: int, hd: int, page_tokens: int, n_splits: int = 4, variant: int = 0) -> torch.Tensor:
+    """q float32 [M][Hq][hd]; kv_bits int16 [n_pages][2][Hkv][page][hd]; page_table int32 [M][max_blocks].
+    variant 0 = standalone kernel, 1 = the units of the persistent decode-step kernel."""
     _require_cuda()
     M = q.shape[0]
     out = torch.empty((M, Hq, hd), dtype=torch.float32, device=q.device)
     _check(lib().sagc_debug_attention(q.data_ptr(), kv_bits.data_ptr(), page_table.data_ptr(), ctx.data_ptr(), M, Hq,
-                                      Hkv, hd, page_tokens, page_table.shape[1], out.data_ptr(), _stream()))
+                                      Hkv, hd, page_tokens, page_table.shape[1], n_splits, variant, out.data_ptr(),
+                                      _stream()))
     return out

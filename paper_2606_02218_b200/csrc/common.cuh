@@ -54,6 +54,21 @@ __device__ __forceinline__ void prefetch_l2(const void* p) {
     asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p));
 }
 
+// ---- Philox4x32-10 (published round function; reading C2) -- the ONE device copy, used by the
+// standalone sampler (sampler.cu) and by the fused LM-head epilogue (tc_linear.cu) ------------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                              uint32_t k1, uint32_t (&out)[4]) {
+#pragma unroll
+    for (int i = 0; i < 10; ++i) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
 // Gumbel draw of the sampler from one Philox word (step a12):  u = ((x >> 9) + 0.5) * 2^-23,  g = -log(-log u).
 // Two MUFU.LG2 instead of two full-range logf: the inner log is taken as the series of -log(1 - e) with
 // e = 1 - u formed EXACTLY when u is within 2^-6 of 1 (that is where the largest draws -- the likely winners

@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <vector>
+
 namespace sagc {
 
 typedef uint16_t bf16_t;   // raw bf16 bit pattern
@@ -173,5 +175,37 @@ int launch_pick_candidates(const float* part_score, const int* part_tok, int n_p
 int launch_embed_split(const bf16_t* embed, const int* tok, const int* m_dev, int m_max, int d, float* x,
                        const bf16_t* norm_w, bf16_t* xs, float* ssq, int ssq_ld, int ssq_tiles, cudaStream_t st);
 int launch_split_rows(const float* x, int K, const int* m_dev, int m_max, bf16_t* xs, cudaStream_t st);
+
+// ---- persistent decode-step kernel (decode_step.cu) ----------------------------------------------
+static constexpr int STEP_KS_MAX = 16;                        // widest K split of one output tile
+struct StepSeg { int tile, kb0, kb1, rank, ks, slot0, pad0, pad1; };   // one unit: weight tile x k blocks [kb0, kb1)
+struct StepPhasePlan { int nseg, pad[3]; StepSeg seg[2]; };   // the units of one CTA in one GEMM phase
+struct StepGemm { int K, n_kb, tiles, na, seg0_tiles, seg1_tiles, tile_ctr_off, ks; };   // phases: 0 QKV, 1 O, 2 gate/up, 3 down
+struct StepLaunch {
+    int n_layers, n_cta, n_slots, m_max;
+    StepGemm g[4];
+    const void* wmaps_dev;                  // device CUtensorMap [n_layers][7]
+    const StepPhasePlan* plan_dev;          // device [4][n_cta]
+    const TcMap (*bmaps)[4];                // host: {xs, att_s, act_s} x UMMA N {32, 64, 128, 256}
+    float* x; float* qkv; bf16_t* xs; bf16_t* att_s; bf16_t* act_s; float* ssq;
+    int ssq_ld, d_tiles, d_model, Nqkv, qd, d_ff;
+    const bf16_t* const* norm1_dev; const bf16_t* const* norm2_dev; const bf16_t* final_norm; const bf16_t* embed;
+    float eps;
+    float* scratch;                         // >= 2 * n_cta * 2 * 64 * 128 floats
+    unsigned* sync_base; int gbar_n, tcnt_n, tiles_per_layer;
+    const int* live; const int* pos; const int* ctx; const int* tok; const int* n_live; const int* step;
+    AttnArgs att;                           // everything but kv_layer / kv_layer_w (set per layer in the kernel)
+    bf16_t* kv_pool; size_t layer_stride;
+    int* err;
+    unsigned long long* trace;              // optional in-kernel timeline (SAGC_STEP_TRACE=1), else null
+    bool cooperative, pdl;
+};
+int launch_decode_step(const StepLaunch& s, cudaStream_t st);
+// static unit -> CTA schedule of the four GEMM phases of a layer; false if the shape does not fit (<= 2 units per CTA and phase)
+bool build_step_plan(int n_cta, int d_model, int qd, int kvd, int d_ff, StepGemm g[4], std::vector<StepPhasePlan>& plan,
+                     int* tiles_per_layer);
+int step_smem_bytes(int n_slots);
+int launch_attention_units(const AttnArgs& a, int n_cta, cudaStream_t st);   // parity entry: head_dim 64 / 128
+int step_ring_slots(int smem_limit);
 
 }  // namespace sagc

@@ -106,6 +106,14 @@ struct sagc_model {
     int ssq_ld, d_tiles;
     std::vector<TcMap> wmaps;                  // per layer: q k v o g u d ; last = lm_head
     TcMap amaps[3][4];                         // {xs, att_s, act_s} x UMMA N {32, 64, 128, 256}
+    // persistent decode-step kernel (decode_step.cu): static work plan, device copies of the per-layer tables, counters
+    bool step_ok; int n_sm, step_slots, gbar_n, tcnt_n, tiles_per_layer;
+    StepGemm step_g[4];
+    void* wmaps_d; StepPhasePlan* plan_d; const bf16_t** norm1_d; const bf16_t** norm2_d; unsigned* step_sync; int* step_err;
+    bool step_coop;
+    unsigned long long* step_trace;            // SAGC_STEP_TRACE=1: in-kernel timeline of one decode step (sagc_debug_step_trace)
+    // host-buffer entry point: device staging buffers, grown on demand and kept by the handle
+    int *h_prompt, *h_tok, *h_len, *h_stats; float* h_ratio; size_t h_prompt_cap, h_tok_cap, h_len_cap, h_grp_cap;
     cudaStream_t own_stream;                   // used when the caller passes the legacy default stream
     cudaEvent_t own_event;
 };
@@ -190,6 +198,9 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     m->tok_cap = m->forced_cap = m->dump_cap = m->prompt_cap = 0;
     m->row_cap = 0;
     m->row_sid = m->row_pos = m->row_ctx = m->row_tok = nullptr;
+    m->h_prompt = m->h_tok = m->h_len = m->h_stats = nullptr; m->h_ratio = nullptr;
+    m->h_prompt_cap = m->h_tok_cap = m->h_len_cap = m->h_grp_cap = 0;
+    m->step_ok = false; m->n_sm = 0; m->step_trace = nullptr;
 
     DA(m->kv_pool, m->layer_stride * (size_t)(L > 0 ? L : 1));
     // RoPE table: angle = pos * theta^(-2i/hd) and cos/sin in fp64 on the host, stored as fp32
@@ -268,6 +279,36 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
                 bad |= tc_make_map(&m->amaps[2][i], m->act_s, 2 * (long long)Rp, c.d_ff, 32 << i);
             }
             if (bad) { sagc_model_destroy(m); return set_err(SAGC_ECUDA, "cuTensorMapEncodeTiled failed"); }
+        }
+        // persistent decode-step kernel: one CTA per SM, static unit -> CTA plan, tensor maps / norm gains in device tables
+        m->step_ok = false; m->wmaps_d = nullptr; m->plan_d = nullptr; m->norm1_d = m->norm2_d = nullptr; m->step_sync = nullptr; m->step_err = nullptr;
+        {
+            int dev = 0, smem_optin = 0;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&m->n_sm, cudaDevAttrMultiProcessorCount, dev);
+            cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+            m->step_slots = step_ring_slots(smem_optin);
+            m->step_coop = env_int("SAGC_STEP_COOP", 1) != 0;
+            std::vector<StepPhasePlan> plan;
+            if (m->tc_ok && env_int("SAGC_STEP", 1) != 0 && c.head_dim >= 64 && m->n_sm > 0 && m->step_slots >= 4 &&
+                build_step_plan(m->n_sm, c.d_model, qd, kvd, c.d_ff, m->step_g, plan, &m->tiles_per_layer)) {
+                m->gbar_n = 1 + 5 * L; m->tcnt_n = m->tiles_per_layer * L;
+                unsigned char* wm = nullptr;
+                DA(wm, (size_t)L * 7 * sizeof(TcMap)); m->wmaps_d = wm;
+                DA(m->plan_d, plan.size()); DA(m->norm1_d, L); DA(m->norm2_d, L);
+                DA(m->step_sync, (size_t)2 * (m->gbar_n + m->tcnt_n)); DA(m->step_err, 1);
+                cudaMemcpy(m->wmaps_d, m->wmaps.data(), (size_t)L * 7 * sizeof(TcMap), cudaMemcpyHostToDevice);
+                cudaMemcpy(m->plan_d, plan.data(), plan.size() * sizeof(StepPhasePlan), cudaMemcpyHostToDevice);
+                cudaMemcpy(m->norm1_d, m->norm1.data(), L * sizeof(void*), cudaMemcpyHostToDevice);
+                cudaMemcpy(m->norm2_d, m->norm2.data(), L * sizeof(void*), cudaMemcpyHostToDevice);
+                cudaMemset(m->step_sync, 0, (size_t)2 * (m->gbar_n + m->tcnt_n) * sizeof(unsigned));
+                cudaMemset(m->step_err, 0, sizeof(int));
+                m->step_ok = true;
+                if (env_int("SAGC_STEP_TRACE", 0)) {
+                    DA(m->step_trace, 2 + 2 * 16000);
+                    cudaMemset(m->step_trace, 0, (2 + 2 * 16000) * sizeof(unsigned long long));
+                }
+            }
         }
     }
     cudaError_t e = cudaDeviceSynchronize();
@@ -476,12 +517,40 @@ static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
 // ---------------------------------------------------------------------------------------
 // sagc_rollout_group
 // ---------------------------------------------------------------------------------------
+// the persistent decode-step kernel covers the tcgen05 path at <= 64 live rows (head_dim 64 / 128)
+static bool step_kernel_applies(const sagc_model* m, int kind, int m_bucket) {
+    return m->step_ok && kind == LIN_TC && m_bucket <= 64 && m->skip_mask == 0;
+}
+
 static int enqueue_decode_step(sagc_model* m, const RolloutDev& rd, int m_bucket, int n_splits, int kind,
                                int n_dump, float* dump_out, cudaStream_t st) {
     RowSet rs = {m->ps.live, m->ps.pos, m->ps.ctx, m->ps.tok, m->ps.n_live, m_bucket};
-    int n = enqueue_layers(m, rs, n_splits, kind, st);
-    if (n < 0) return -1;
     const sagc_model_config& c = m->cfg;
+    int n;
+    if (step_kernel_applies(m, kind, m_bucket)) {
+        // a5 - a10 of every layer in ONE persistent kernel (decode_step.cu)
+        StepLaunch s = {};
+        s.n_layers = c.n_layers; s.n_cta = m->n_sm; s.n_slots = m->step_slots; s.m_max = m_bucket;
+        for (int i = 0; i < 4; ++i) s.g[i] = m->step_g[i];
+        s.wmaps_dev = m->wmaps_d; s.plan_dev = m->plan_d; s.bmaps = m->amaps;
+        s.x = m->x; s.qkv = m->qkv; s.xs = m->xs; s.att_s = m->att_s; s.act_s = m->act_s; s.ssq = m->ssq;
+        s.ssq_ld = m->ssq_ld; s.d_tiles = m->d_tiles; s.d_model = c.d_model; s.Nqkv = m->Nqkv; s.qd = c.n_q_heads * c.head_dim; s.d_ff = c.d_ff;
+        s.norm1_dev = m->norm1_d; s.norm2_dev = m->norm2_d; s.final_norm = m->final_norm; s.embed = m->embed; s.eps = c.rms_eps;
+        s.scratch = m->tc_scratch; s.sync_base = m->step_sync; s.gbar_n = m->gbar_n; s.tcnt_n = m->tcnt_n; s.tiles_per_layer = m->tiles_per_layer;
+        s.live = m->ps.live; s.pos = m->ps.pos; s.ctx = m->ps.ctx; s.tok = m->ps.tok; s.n_live = m->ps.n_live; s.step = m->ps.step;
+        AttnArgs& aa = s.att;
+        aa.q = m->qkv; aa.ldq = m->Nqkv; aa.page_table = m->ps.page_table; aa.max_blocks = m->max_blocks; aa.row_sid = m->ps.live;
+        aa.row_ctx = m->ps.ctx; aa.m_dev = m->ps.n_live; aa.m_max = m_bucket; aa.Hq = c.n_q_heads; aa.Hkv = c.n_kv_heads; aa.hd = c.head_dim;
+        aa.page = c.page_tokens; aa.n_splits = 1; aa.part_o = m->part_o; aa.part_ml = m->part_ml; aa.counters = m->counters; aa.out = m->att;
+        aa.out_split = m->att_s; aa.ld_split = c.n_q_heads * c.head_dim; aa.fuse_rope = 1; aa.rope_cs = m->rope_cs; aa.row_pos = m->ps.pos;
+        aa.prefetch = 0; aa.cluster_merge = 0;
+        s.kv_pool = m->kv_pool; s.layer_stride = m->layer_stride; s.err = m->step_err; s.trace = m->step_trace;
+        s.cooperative = m->step_coop; s.pdl = m->use_pdl && !m->step_coop;
+        n = launch_decode_step(s, st);
+    } else {
+        n = enqueue_layers(m, rs, n_splits, kind, st);
+    }
+    if (n < 0) return -1;
     if (m->lm_fused && kind == LIN_TC && m_bucket <= 64 && n_dump == 0 && (c.vocab % 128) == 0 && !(m->skip_mask & (2 | 16))) {
         // a11 + a12 in one persistent kernel: the logits never reach HBM
         LmSampleArgs f = {};
@@ -691,6 +760,7 @@ extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, c
     int cur_phase = -1;
     cudaEvent_t ph_start[3] = {nullptr, nullptr, nullptr}, ph_end[3] = {nullptr, nullptr, nullptr};
     int live_bound = nseq;
+    bool prev_mega = false;
     int t = 2;
     while (true) {
         int live;
@@ -727,8 +797,12 @@ extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, c
             launches += launch_advance(m->ps, rd, m->part_score, m->sampled, 1, st);
         } else {
             const int mb = round_bucket(live);
-            const int ns = pick_splits(m, mb, pmax + t - 1);
             const int kind = pick_kind(m, prm->path, mb);
+            const bool mega = step_kernel_applies(m, kind, mb);
+            const int ns = mega ? 0 : pick_splits(m, mb, pmax + t - 1);      // the step kernel picks its K-splits on the device
+            if (mega && !prev_mega)       // both counter sets must be clear when the step kernel takes over
+                CU(cudaMemsetAsync(m->step_sync, 0, (size_t)2 * (m->gbar_n + m->tcnt_n) * sizeof(unsigned), st));
+            prev_mega = mega;
             if (use_graph) {
                 GraphKey key = {mb, ns, kind, prm->n_dump};
                 auto it = m->graphs.find(key);
@@ -899,6 +973,23 @@ extern "C" int sagc_debug_peak_pages(sagc_model* m, int32_t* peak) {
     CU(cudaMemcpy(peak, m->ps.peak_used, sizeof(int), cudaMemcpyDeviceToHost));
     return SAGC_OK;
 }
+extern "C" int sagc_debug_step_trace(sagc_model* m, int64_t record_step, uint64_t* out, int32_t capacity, int32_t* n) {
+    if (!m || !n) return set_err(SAGC_EINVAL, "null argument");
+    *n = 0;
+    if (!m->step_trace) return SAGC_OK;                      // tracing is off (SAGC_STEP_TRACE unset at model create)
+    CU(cudaDeviceSynchronize());
+    unsigned long long hdr[2];
+    CU(cudaMemcpy(hdr, m->step_trace, sizeof(hdr), cudaMemcpyDeviceToHost));
+    int k = (int)(hdr[1] < 16000ull ? hdr[1] : 16000ull);
+    if (out) {
+        if (k > capacity) k = capacity;
+        CU(cudaMemcpy(out, m->step_trace + 2, (size_t)k * 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+        *n = k;
+    }
+    hdr[0] = (unsigned long long)record_step; hdr[1] = 0;    // arm the next recording
+    CU(cudaMemcpy(m->step_trace, hdr, sizeof(hdr), cudaMemcpyHostToDevice));
+    return SAGC_OK;
+}
 extern "C" int sagc_debug_philox(uint64_t seed, int32_t sid, int32_t t, int32_t v0, int32_t n, uint32_t* out, void* stream) {
     if (n < 0 || (n > 0 && !out)) return set_err(SAGC_EINVAL, "null argument");
     launch_philox_debug(seed, sid, t, v0, n, out, reinterpret_cast<cudaStream_t>(stream));
@@ -993,12 +1084,14 @@ extern "C" int sagc_debug_lm_sample(const void* W, const float* x, int32_t M, in
     return SAGC_OK;
 }
 extern "C" int sagc_debug_attention(const float* q, const void* kv, const int32_t* page_table, const int32_t* ctx, int32_t M,
-                                    int32_t Hq, int32_t Hkv, int32_t hd, int32_t page_tokens, int32_t max_blocks, float* out,
-                                    void* stream) {
+                                    int32_t Hq, int32_t Hkv, int32_t hd, int32_t page_tokens, int32_t max_blocks, int32_t n_splits,
+                                    int32_t variant, float* out, void* stream) {
     if (!q || !kv || !page_table || !ctx || !out || M < 1) return set_err(SAGC_EINVAL, "null argument");
     if (Hq % Hkv || Hq / Hkv > 8) return set_err(SAGC_EINVAL, "bad head counts");
+    if (n_splits < 1 || n_splits > 64) return set_err(SAGC_EINVAL, "n_splits must be in 1..64");
+    if (variant != 0 && variant != 1) return set_err(SAGC_EINVAL, "variant must be 0 (standalone kernel) or 1 (decode-step units)");
+    if (variant == 1 && hd != 64 && hd != 128) return set_err(SAGC_EINVAL, "the decode-step units need head_dim 64 or 128");
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    const int n_splits = env_int("SAGC_DEBUG_SPLITS", 4);
     int *sid = nullptr, *cnt = nullptr;
     float *po = nullptr, *pml = nullptr;
     CU(cudaMalloc(&sid, M * sizeof(int)));
@@ -1013,7 +1106,9 @@ extern "C" int sagc_debug_attention(const float* q, const void* kv, const int32_
     a.q = q; a.ldq = Hq * hd; a.kv_layer = reinterpret_cast<const bf16_t*>(kv); a.page_table = page_table;
     a.max_blocks = max_blocks; a.row_sid = sid; a.row_ctx = ctx; a.m_dev = nullptr; a.m_max = M; a.Hq = Hq; a.Hkv = Hkv;
     a.hd = hd; a.page = page_tokens; a.n_splits = n_splits; a.part_o = po; a.part_ml = pml; a.counters = cnt; a.out = out;
-    int r = launch_attention(a, st);
+    int n_sm = 148;
+    { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); }
+    int r = variant == 1 ? launch_attention_units(a, n_sm, st) : launch_attention(a, st);
     cudaError_t e = cudaStreamSynchronize(st);
     cudaFree(sid); cudaFree(cnt); cudaFree(po); cudaFree(pml);
     if (r < 0) return set_err(SAGC_EINVAL, "unsupported head_dim %d", hd);

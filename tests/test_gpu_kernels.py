@@ -150,13 +150,10 @@ def test_fused_lm_head_sampler_vs_oracle(B, monkeypatch, M, V, K, ctas, mode):
 
 
 # ---------------------------------------------------------------------------- a7
-@pytest.mark.parametrize("Hq,Hkv,hd,page", [(4, 4, 32, 16), (14, 2, 64, 64), (28, 4, 128, 64), (8, 1, 128, 32)])
-def test_paged_attention_vs_fp64(B, Hq, Hkv, hd, page):
-    rng = np.random.default_rng(Hq * 100 + hd)
-    ctxs = np.array([1, 2, page - 1, page, page + 1, 127, 128, 129, 700, 1500], dtype=np.int32)
+def _attention_case(rng, ctxs, Hq, Hkv, hd, page):
     M = len(ctxs)
     max_blocks = (int(ctxs.max()) + page - 1) // page
-    n_pages = M * max_blocks + 3
+    n_pages = int(sum((int(c) + page - 1) // page for c in ctxs)) + 3
     perm = rng.permutation(n_pages)
     pt = -np.ones((M, max_blocks), dtype=np.int32)
     k = 0
@@ -176,5 +173,29 @@ def test_paged_attention_vs_fp64(B, Hq, Hkv, hd, page):
             s = K[h // r] @ q[m, h].astype(np.float64) / np.sqrt(hd)
             p = np.exp(s - s.max()); p /= p.sum()
             ref[m, h] = p @ V[h // r]
-    out = B.debug_attention(_dev(q), _dev(kv.view(np.int16)), _dev(pt), _dev(ctxs), Hq, Hkv, hd, page).cpu().numpy()
+    return q, kv, pt, ref
+
+
+@pytest.mark.parametrize("Hq,Hkv,hd,page", [(4, 4, 32, 16), (14, 2, 64, 64), (28, 4, 128, 64), (8, 1, 128, 32)])
+@pytest.mark.parametrize("splits,variant", [(1, 0), (2, 0), (4, 0), (8, 0), (16, 0), (1, 1), (3, 1), (8, 1), (32, 1)])
+def test_paged_attention_vs_fp64(B, Hq, Hkv, hd, page, splits, variant):
+    """variant 0: the standalone kernel (cluster merge for 2..8 splits, L2 merge for 16); variant 1: the units of the
+    persistent decode-step kernel (its tile geometry, unit loop and last-arriver merge)."""
+    if variant == 1 and hd == 32:
+        pytest.skip("the decode-step kernel serves head_dim 64 / 128")
+    rng = np.random.default_rng(Hq * 100 + hd)
+    ctxs = np.array([1, 2, page - 1, page, page + 1, 127, 128, 129, 700, 1500], dtype=np.int32)
+    q, kv, pt, ref = _attention_case(rng, ctxs, Hq, Hkv, hd, page)
+    out = B.debug_attention(_dev(q), _dev(kv.view(np.int16)), _dev(pt), _dev(ctxs), Hq, Hkv, hd, page, splits, variant).cpu().numpy()
+    assert np.max(np.abs(out - ref)) < 2e-5, np.max(np.abs(out - ref))
+
+
+@pytest.mark.parametrize("Hq,Hkv,hd", [(14, 2, 64), (28, 4, 128)])
+@pytest.mark.parametrize("splits,variant", [(1, 0), (2, 0), (4, 0), (8, 0), (16, 0), (1, 1), (8, 1), (18, 1), (32, 1)])
+def test_paged_attention_long_context(B, Hq, Hkv, hd, splits, variant):
+    """The contexts of the full-size configs: 4 095 / 4 352 (cfg2 cap), 8 704 (cfg3/4 cap), 17 408 (cfg5 cap)."""
+    rng = np.random.default_rng(hd + splits)
+    ctxs = np.array([4095, 4352, 8704, 17408], dtype=np.int32)
+    q, kv, pt, ref = _attention_case(rng, ctxs, Hq, Hkv, hd, 64)
+    out = B.debug_attention(_dev(q), _dev(kv.view(np.int16)), _dev(pt), _dev(ctxs), Hq, Hkv, hd, 64, splits, variant).cpu().numpy()
     assert np.max(np.abs(out - ref)) < 2e-5, np.max(np.abs(out - ref))
