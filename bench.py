@@ -82,30 +82,69 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_sample(w, weights, n_steps=1):
-    """The CPU oracle, as it stands, on a bounded slice of the same workload: 1 prompt of 64 tokens,
-    G = 8 completions, 8 generated tokens each (64 tokens/step).  Returns (tokens/s, cores, text)."""
-    from oracle import decoder as odec, rollout as oro
-    import torch
-    dec = odec.RefDecoder(w.model, weights)
-    prompts, offs = wl.make_prompts(w, n_prompts=1, prompt_len=64)
-    G, max_new = 8, 8
-    mode = 1 if w.sampling == "gumbel" else 0
-    t0 = time.perf_counter()
-    n_tok = 0
-    for _ in range(n_steps):
-        res = oro.rollout_group(dec, prompts, offs, G, mode, w.temperature, w.philox_seed, max_new)
-        n_tok += int(res.lengths.sum())
-    dt = time.perf_counter() - t0
-    cores = torch.get_num_threads() if hasattr(torch, "get_num_threads") else os.cpu_count()
+SLICE_PREFILL, SLICE_CTX, SLICE_ROWS, SLICE_STEPS = 64, 512, 8, 8
+
+
+def _blas_threads():
     try:
         from threadpoolctl import threadpool_info
         nt = [p["num_threads"] for p in threadpool_info() if p.get("user_api") == "blas"]
         if nt:
-            cores = max(nt)
+            return int(max(nt))
     except Exception:
         pass
-    return n_tok / dt, int(cores), "1 prompt x 64 tokens prefill, G=8, 8 generated tokens each (numpy fp32 oracle)"
+    return int(os.cpu_count() or 1)
+
+
+def oracle_slice(w, weights, single_thread=False):
+    """The CPU oracle, as it stands, on the slice BASELINE.md section 4 plans: one 64-token prefill (timed on its
+    own), then SLICE_STEPS decode steps of SLICE_ROWS sequences whose context grows to SLICE_CTX.  The cache is set
+    up by an (untimed) oracle prefill of SLICE_CTX - SLICE_STEPS tokens forked SLICE_ROWS ways.
+    Returns {decode tokens/s, prefill tokens/s, threads}."""
+    from oracle import decoder as odec, philox as oph
+    from contextlib import nullcontext
+    try:
+        from threadpoolctl import threadpool_limits
+        lim = threadpool_limits(limits=1) if single_thread else nullcontext()
+    except Exception:
+        lim = nullcontext()
+    with lim:
+        dec = odec.RefDecoder(w.model, weights)
+        P0 = SLICE_CTX - SLICE_STEPS
+        prompts, _ = wl.make_prompts(w, n_prompts=1, prompt_len=P0)
+        mode = 1 if w.sampling == "gumbel" else 0
+        t0 = time.perf_counter()
+        dec.prefill(prompts[:SLICE_PREFILL])
+        t_pf = time.perf_counter() - t0
+        threads = 1 if single_thread else _blas_threads()
+        lg, cache = dec.prefill(prompts)                      # untimed: brings the cache to context SLICE_CTX - SLICE_STEPS
+        caches = [dec.fork_cache(cache) for _ in range(SLICE_ROWS)]
+        toks = [oph.sample_token(lg, mode, w.temperature, w.philox_seed, g, 1) for g in range(SLICE_ROWS)]
+        t0 = time.perf_counter()
+        for t in range(2, SLICE_STEPS + 2):
+            for g in range(SLICE_ROWS):
+                lg = dec.step(toks[g], P0 + t - 2, caches[g])
+                toks[g] = oph.sample_token(lg, mode, w.temperature, w.philox_seed, g, t)
+        dt = time.perf_counter() - t0
+    return {"decode_tokens_per_s": SLICE_ROWS * SLICE_STEPS / dt, "prefill_tokens_per_s": SLICE_PREFILL / t_pf, "threads": threads}
+
+
+SLICE_TEXT = (f"{SLICE_PREFILL}-token prefill (timed on its own), then {SLICE_STEPS} decode steps of {SLICE_ROWS} sequences at "
+              f"context {SLICE_CTX - SLICE_STEPS + 1}..{SLICE_CTX} (BASELINE.md section 4); numpy fp32 oracle")
+
+
+def gpu_slice(B, make_model, w):
+    """The GPU on the identical slice: 1 prompt of SLICE_CTX - SLICE_STEPS tokens, G = SLICE_ROWS, SLICE_STEPS decode steps."""
+    P0 = SLICE_CTX - SLICE_STEPS
+    prompts, offs = wl.make_prompts(w, n_prompts=1, prompt_len=P0)
+    m = make_model(64, SLICE_ROWS, SLICE_CTX + 8)
+    mode = B.MODE_GUMBEL if w.sampling == "gumbel" else B.MODE_GREEDY
+    fl = np.full(SLICE_ROWS, SLICE_STEPS + 1, np.int32)
+    for _ in range(3):
+        out = m.rollout_group(prompts, offs, SLICE_ROWS, mode=mode, temperature=w.temperature, seed=w.philox_seed,
+                              max_new_tokens=SLICE_STEPS + 1, forced_lengths=fl, timing=True)
+    m.close()
+    return SLICE_ROWS * SLICE_STEPS / (out.timing["decode_ms"] * 1e-3)
 
 
 def run_reference(args, rank, world):
@@ -115,14 +154,16 @@ def run_reference(args, rank, world):
     w = wl.WORKLOADS[args.cfg]
     weights = wl.make_weights(w.model, 0)
     for _ in range(args.warmup and 1):
-        oracle_sample(w, weights, 1)
+        oracle_slice(w, weights)
     t0 = time.perf_counter()
-    tps, cores, sample = oracle_sample(w, weights, args.steps)
+    acc = [oracle_slice(w, weights) for _ in range(max(args.steps, 1))]
     dt = time.perf_counter() - t0
+    tps = float(np.mean([a["decode_tokens_per_s"] for a in acc]))
+    cores, sample = acc[0]["threads"], SLICE_TEXT
     line = {"impl": "reference", "metric": METRIC, "value": tps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32 (bf16 weights widened)", "data": "synthetic",
-            "config": {"workload": f"configs[{args.cfg - 1}] (0.5B-shaped decoder) -- bounded sample", "sample": sample},
+            "config": {"workload": f"configs[{args.cfg - 1}] ({SHAPE_NAMES.get(args.cfg, '?')}-shaped decoder) -- bounded sample", "sample": sample},
             "cpu_baseline": {"value": tps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": tps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
@@ -147,44 +188,121 @@ def decode_weight_bytes(mc):
     return 2 * (mc.n_layers * (mc.d_model * q + 2 * mc.d_model * kv + q * mc.d_model + 3 * mc.d_model * mc.d_ff) + mc.vocab * mc.d_model)
 
 
-def kernel_roofline(B, torch, mc, peak):
-    """Time the largest single launch of a decode step alone (LM head, M = 64): CUDA events on the
-    launching stream, weights (272 MB) larger than L2 so every iteration streams from HBM."""
-    rng = np.random.default_rng(1)
-    N, K, M = mc.vocab, mc.d_model, 64
-    W = torch.from_numpy(rng.integers(0, 2 ** 15, size=(N, K), dtype=np.int64).astype(np.int16)).cuda()
-    x = torch.randn(M, K, device="cuda")
-    for _ in range(3):
-        B.debug_linear(W, x, B.PATH_GEMM)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    n = 20
-    e0.record()
-    for _ in range(n):
-        B.debug_linear(W, x, B.PATH_GEMM)
-    e1.record()
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / n
-    nbytes = N * K * 2 + M * K * 4 + M * N * 4
-    out = {"kernel": "k_linear_tc<128,STORE> (LM head, 64 live rows; + k_split_rows)", "bytes": nbytes, "ms": ms,
-           "achieved_gbs": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peak}
-    # the launch the decode step actually uses at <= 64 live rows: LM head + Gumbel sampler fused (logits never stored)
-    sids = torch.arange(M, dtype=torch.int32, device="cuda")
-    for _ in range(3):
-        B.debug_lm_sample(W, x, sids, 5, seed=7)
-    torch.cuda.synchronize()
-    e0.record()
-    for _ in range(n):
-        B.debug_lm_sample(W, x, sids, 5, seed=7)
-    e1.record()
-    torch.cuda.synchronize()
-    ms2 = e0.elapsed_time(e1) / n
-    nb2 = N * K * 2 + M * K * 4
-    out["fused"] = {"kernel": "k_lmhead_sample<128> (persistent LM head + Philox Gumbel arg-max, 64 live rows; + k_split_rows, k_pick_candidates)",
-                    "bytes": nb2, "ms": ms2, "achieved_gbs": nb2 / ms2 / 1e6, "frac": nb2 / ms2 / 1e6 / peak,
-                    # dram__bytes_read.sum of this kernel at this shape, one launch (profiles/r01_ncu_top_kernels.md)
-                    "traffic": 272578048 if (N, K) == (151936, 896) else None}
+BF16_SUSTAINED_TFLOPS_FALLBACK = 1400.0
+
+
+def measured_bf16_sustained():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f).get("bf16_tflops_sustained", BF16_SUSTAINED_TFLOPS_FALLBACK))
+    return BF16_SUSTAINED_TFLOPS_FALLBACK
+
+
+def pool_pages(w, fl, max_new):
+    """KV pool size: worst case (every completion at the cap) if it fits ~100 GB, else sized for the drawn lengths."""
+    mc, page = w.model, w.model.page_tokens
+    n_pages = w.n_prompts * (w.prompt_len // page + w.G * ((max_new + page - 1) // page + 1)) + 8
+    if n_pages * page * 2 * mc.n_layers * mc.n_kv_heads * mc.head_dim * 2 > 100e9:
+        n_pages = int(np.sum((fl + page - 1) // page + 2)) + w.n_prompts * (w.prompt_len // page + 1) + 8
+    return n_pages
+
+
+def phase_table(acc, n_rollouts, peak, mc=None, tf_sustained=None):
+    """Per-phase numbers from the accumulated sagc_rollout_timing fields."""
+    names = ["full", "mid", "tail"]
+    out = {}
+    for p in range(3):
+        if not acc["ph_steps"][p]:
+            continue
+        ms_step = acc["ph_ms"][p] / acc["ph_steps"][p]
+        gbs = acc["ph_bytes"][p] / acc["ph_ms"][p] / 1e6
+        row = {"decode_steps": acc["ph_steps"][p] // n_rollouts, "avg_live_rows": acc["ph_tok"][p] / acc["ph_steps"][p],
+               "tokens_per_s": acc["ph_tok"][p] / acc["ph_ms"][p] * 1e3, "ms_per_decode_step": ms_step, "achieved_gbs": gbs,
+               "frac_of_measured": gbs / peak, "frac_of_8tbs": gbs / 8000.0}
+        if mc is not None and tf_sustained:
+            # two-term roofline (SURVEY 7 H3): the projections are tensor-bound once the hi/lo MMA work (2 passes x 2 flop per
+            # weight and row) outweighs streaming the weights; the KV scan is HBM-bound either way
+            Wb = decode_weight_bytes(mc)
+            bytes_step = acc["ph_bytes"][p] / acc["ph_steps"][p]
+            t_w = Wb / (peak * 1e9)
+            t_mma = 2.0 * 2.0 * (Wb / 2.0) * row["avg_live_rows"] / (tf_sustained * 1e12)
+            t_two = max(t_w, t_mma) + (bytes_step - Wb) / (peak * 1e9)
+            row["two_term_roofline_ms"] = t_two * 1e3
+            row["frac_of_two_term"] = t_two * 1e3 / ms_step
+            row["bound"] = "tensor" if t_mma > t_w else "hbm"
+        out[names[p]] = row
     return out
+
+
+def accumulate(acc, t):
+    acc["tokens"] += t["total_tokens"]; acc["launches"] += t["kernel_launches"] + 1
+    acc["prefill_ms"] += t["prefill_ms"]; acc["prefill_flops"] += t["prefill_flops"]; acc["decode_ms"] += t["decode_ms"]
+    for p in range(3):
+        acc["ph_ms"][p] += t["phase_ms"][p]; acc["ph_bytes"][p] += t["phase_bytes"][p]
+        acc["ph_tok"][p] += t["phase_tokens"][p]; acc["ph_steps"][p] += t["phase_steps"][p]
+
+
+def new_acc():
+    return {"tokens": 0, "launches": 0, "ph_ms": [0.0] * 3, "ph_bytes": [0.0] * 3, "ph_tok": [0] * 3, "ph_steps": [0] * 3,
+            "prefill_ms": 0.0, "prefill_flops": 0.0, "decode_ms": 0.0}
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch from `ncu --set full` (profiles/r02_ncu_top_kernels.md), by shape
+NCU_TRAFFIC = {}
+
+
+def kernel_parts(model, B, w, d_prompts, offs, fl, max_new, mode, peak):
+    """The three parts of a decode step timed alone with CUDA events on the launching stream (SAGC_FLAG_TIME_KERNELS: direct
+    launches instead of graphs, four events per step): layer stack (the persistent decode-step kernel while <= 64 rows are
+    live), LM head + sampler, advance.  Algorithmic bytes of a part = the weights it streams (+ the KV scan for the layer stack)."""
+    mc = w.model
+    out = model.rollout_group(d_prompts, offs, w.G, mode=mode, temperature=w.temperature, seed=w.philox_seed,
+                              max_new_tokens=max_new, forced_lengths=fl, timing=True, flags=B.FLAG_TIME_KERNELS)
+    t = out.timing
+    steps = max(t["kernel_steps"], 1)
+    W = decode_weight_bytes(mc)
+    W_lm = 2 * mc.vocab * mc.d_model
+    bytes_all = sum(t["phase_bytes"])
+    ms = t["kernel_ms"]
+    parts = {}
+    for name, k, nbytes in (("layer_stack", 0, bytes_all - steps * W_lm), ("lm_head_sampler", 1, steps * W_lm), ("advance", 2, 0.0)):
+        parts[name] = {"ms_per_step": ms[k] / steps, "share_of_step": ms[k] / max(sum(ms), 1e-9), "bytes_per_step": nbytes / steps,
+                       "achieved_gbs": nbytes / ms[k] / 1e6 if ms[k] > 0 else None,
+                       "frac": nbytes / ms[k] / 1e6 / peak if ms[k] > 0 else None}
+    parts["layer_stack"]["kernel"] = "k_decode_step (persistent, one launch per step) while <= 64 rows are live; per-layer k_linear_tc / k_attention above"
+    parts["lm_head_sampler"]["kernel"] = "k_lmhead_sample (fused, <= 64 rows) / k_linear_tc + k_sample above"
+    parts["advance"]["kernel"] = "k_advance"
+    parts["steps_measured"] = steps
+    parts["note"] = "direct launches (no CUDA graph) so that events can bracket each part; shares, not absolutes, carry over to the graph run"
+    return parts
+
+
+def side_7b(B, torch, peak, tf_sustained, device):
+    """configs[4] (7B shape, 8 prompts x 1024 x G=32, Pareto lengths capped at 16384) once, after one warm-up rollout."""
+    w = wl.WORKLOADS[5]
+    mc = w.model
+    weights = wl.make_weights(mc, 0)
+    prompts, offs = wl.make_prompts(w)
+    fl = np.minimum(wl.make_forced_lengths(w), w.max_new).astype(np.int32)
+    model = B.Model(mc, weights, pool_pages(w, fl, w.max_new), w.n_prompts * w.G, w.prompt_len + w.max_new, device=device)
+    del weights
+    d_prompts = torch.from_numpy(prompts).cuda()
+    mode = B.MODE_GUMBEL
+    acc = new_acc()
+    for it in range(2):
+        out = model.rollout_group(d_prompts, offs, w.G, mode=mode, temperature=w.temperature, seed=w.philox_seed,
+                                  max_new_tokens=w.max_new, forced_lengths=fl, timing=True)
+    accumulate(acc, out.timing)
+    model.close()
+    dec_bytes, dec_ms = sum(acc["ph_bytes"]), sum(acc["ph_ms"])
+    return {"workload": "configs[4]: 7B-shaped decoder, 8 prompts x 1024 tokens x G=32, forced lengths pareto(512, 1.5) cap 16384, Gumbel T=1 Philox",
+            "rollouts": "1 warm-up + 1 timed", "tokens": acc["tokens"], "tokens_per_s": acc["tokens"] / (out.timing["prefill_ms"] + out.timing["decode_ms"]) * 1e3,
+            "decode_achieved_gbs": dec_bytes / dec_ms / 1e6, "decode_frac_of_measured": dec_bytes / dec_ms / 1e6 / peak,
+            "decode_frac_of_8tbs": dec_bytes / dec_ms / 1e6 / 8000.0,
+            "phases": phase_table(acc, 1, peak, mc, tf_sustained),
+            "prefill": {"ms": acc["prefill_ms"], "tflops_model": acc["prefill_flops"] / acc["prefill_ms"] / 1e9 if acc["prefill_ms"] else None},
+            "targets": {"full_frac_of_8tbs": 0.70, "tail_frac_of_8tbs": 0.60}}
 
 
 def main():
@@ -196,6 +314,7 @@ def main():
     ap.add_argument("--cfg", type=int, default=2)
     ap.add_argument("--max-new", type=int, default=0, help="override max_new_tokens (debug; invalidates the number)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-side-7b", action="store_true", help="skip the configs[4] (7B shape) side block (~5 minutes)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -220,19 +339,15 @@ def main():
     prompts, offs = wl.make_prompts(w)
     fl = np.minimum(wl.make_forced_lengths(w), max_new).astype(np.int32)
     rewards, goffs = wl.make_rewards(w)
-    page = mc.page_tokens
     nseq = w.n_prompts * w.G
-    n_pages = w.n_prompts * (w.prompt_len // page + w.G * ((max_new + page - 1) // page + 1)) + 8
-    if n_pages * page * 2 * mc.n_layers * mc.n_kv_heads * mc.head_dim * 2 > 100e9:
-        # worst case (every completion at the cap) does not fit: size the pool for the forced lengths actually drawn
-        # (an upper bound that needs no retirement: every sequence's own blocks + the shared prefix blocks)
-        n_pages = int(np.sum((fl + page - 1) // page + 2)) + w.n_prompts * (w.prompt_len // page + 1) + 8
-    model = B.Model(mc, weights, n_pages, nseq, w.prompt_len + max_new, device=f"cuda:{local}")
+    model = B.Model(mc, weights, pool_pages(w, fl, max_new), nseq, w.prompt_len + max_new, device=f"cuda:{local}")
     mode = B.MODE_GUMBEL if w.sampling == "gumbel" else B.MODE_GREEDY
     adv_mode = B.ADV_DAPO if w.adv_mode == "DAPO" else B.ADV_GRPO
     d_prompts = torch.from_numpy(prompts).cuda()
     d_rewards, d_goffs = torch.from_numpy(rewards).cuda(), torch.from_numpy(goffs).cuda()
     stream = torch.cuda.Stream()
+    peak, peak_src = measured_peaks()
+    tf_sus = measured_bf16_sustained()
 
     def step(host=False, timing=True):
         out = model.rollout_group(prompts if host else d_prompts, offs, w.G, mode=mode, temperature=w.temperature,
@@ -253,17 +368,11 @@ def main():
         sampler = ClockSampler(local)
         sampler.start()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        acc = {"tokens": 0, "launches": 0, "ph_ms": [0.0] * 3, "ph_bytes": [0.0] * 3, "ph_tok": [0] * 3, "ph_steps": [0] * 3,
-               "prefill_ms": 0.0, "prefill_flops": 0.0, "decode_ms": 0.0}
+        acc = new_acc()
         e0.record()
         for _ in range(args.steps):
             out, adv, keep = step()
-            t = out.timing
-            acc["tokens"] += t["total_tokens"]; acc["launches"] += t["kernel_launches"] + 1
-            acc["prefill_ms"] += t["prefill_ms"]; acc["prefill_flops"] += t["prefill_flops"]; acc["decode_ms"] += t["decode_ms"]
-            for p in range(3):
-                acc["ph_ms"][p] += t["phase_ms"][p]; acc["ph_bytes"][p] += t["phase_bytes"][p]
-                acc["ph_tok"][p] += t["phase_tokens"][p]; acc["ph_steps"][p] += t["phase_steps"][p]
+            accumulate(acc, out.timing)
         e1.record()
         barrier()
         clocks = sampler.stop()
@@ -277,24 +386,20 @@ def main():
             e2e_tok += int(out_h.lengths.sum())
         torch.cuda.synchronize()
         e2e_s = time.perf_counter() - t0
-        peak, peak_src = measured_peaks()
-        kr = kernel_roofline(B, torch, mc, peak) if rank == 0 else None
+        parts = kernel_parts(model, B, w, d_prompts, offs, fl, max_new, mode, peak) if rank == 0 else None
+        gpu_slice_tps = None
+        if rank == 0 and not args.no_cpu_baseline:
+            gpu_slice_tps = gpu_slice(B, lambda n_pages, max_seqs, max_ctx: B.Model(mc, weights, n_pages, max_seqs, max_ctx, device=f"cuda:{local}"), w)
 
     ms, e2e_ms = allreduce_max([ms, e2e_s * 1e3], "cuda", world)
+    model.close()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-    names = ["full", "mid", "tail"]
-    phases = {}
-    for p in range(3):
-        if acc["ph_steps"][p]:
-            gbs = acc["ph_bytes"][p] / acc["ph_ms"][p] / 1e6
-            phases[names[p]] = {"decode_steps": acc["ph_steps"][p] // args.steps, "tokens_per_s": acc["ph_tok"][p] / acc["ph_ms"][p] * 1e3,
-                                "ms_per_decode_step": acc["ph_ms"][p] / acc["ph_steps"][p], "achieved_gbs": gbs,
-                                "frac_of_measured": gbs / peak, "frac_of_8tbs": gbs / 8000.0}
     dec_bytes = sum(acc["ph_bytes"]); dec_ms = sum(acc["ph_ms"])
     achieved = dec_bytes / dec_ms / 1e6
+    ls = parts["layer_stack"]
     line = {"metric": METRIC, "value": world * acc["tokens"] / ms * 1e3, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
@@ -307,18 +412,31 @@ def main():
             "clocks": clocks, "gpu_launches": acc["launches"],
             "e2e": {"value": world * e2e_tok / e2e_ms * 1e3, "unit": UNIT, "h2d_bytes_per_step": int(prompts.nbytes + fl.nbytes),
                     "d2h_bytes_per_step": int(nseq * max_new * 4 + nseq * 4 + w.n_prompts * 16)},
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "peak_source": peak_src,
-                         "what": "all decode steps of the rollout (every kernel of the step graph): algorithmic bytes "
-                                 "(weights once + prefix KV once per live group + suffix KV + KV written) / device time",
-                         "frac_of_8tbs": achieved / 8000.0},
-            "phases": phases, "kernel_roofline": kr,
+            # the dominant kernel: the layer stack of a decode step (one persistent launch per step while <= 64 rows are live)
+            "roofline": {"bound": "hbm", "achieved": ls["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": ls["frac"],
+                         "traffic": NCU_TRAFFIC.get((args.cfg, "layer_stack")), "peak_source": peak_src,
+                         "kernel": ls["kernel"], "share_of_decode_step": ls["share_of_step"],
+                         "what": "layer-stack launch of every decode step of one rollout, timed alone with CUDA events on the launching stream "
+                                 "(SAGC_FLAG_TIME_KERNELS): algorithmic bytes (layer weights once + prefix KV once per live group + suffix KV + "
+                                 "KV written) / device time",
+                         "frac_of_8tbs": ls["achieved_gbs"] / 8000.0},
+            "roofline_all_decode": {"achieved": achieved, "frac": achieved / peak, "frac_of_8tbs": achieved / 8000.0,
+                                    "what": "every kernel of every decode step of the timed rollouts (graph launches): algorithmic bytes / device time"},
+            "phases": phase_table(acc, args.steps, peak, mc, tf_sus), "kernel_roofline": parts,
             "prefill": {"ms": acc["prefill_ms"] / args.steps, "tflops": acc["prefill_flops"] / acc["prefill_ms"] / 1e9 if acc["prefill_ms"] else None}}
     if not args.no_cpu_baseline:
-        tps, cores, sample = oracle_sample(w, weights, 1)
-        line["cpu_baseline"] = {"value": tps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        multi = oracle_slice(w, weights)
+        single = oracle_slice(w, weights, single_thread=True)
+        line["cpu_baseline"] = {"value": multi["decode_tokens_per_s"], "unit": UNIT, "cores": multi["threads"], "kind": "oracle",
+                                "sample": SLICE_TEXT, "single_thread_value": single["decode_tokens_per_s"],
+                                "prefill_tokens_per_s": multi["prefill_tokens_per_s"], "gpu_same_slice_tokens_per_s": gpu_slice_tps}
+    del weights
+    if not args.no_side_7b and args.cfg == 2 and world == 1:
+        try:
+            line["side_7b"] = side_7b(B, torch, peak, tf_sus, f"cuda:{local}")
+        except Exception as e:                                   # the side block must never cost the headline line
+            line["side_7b"] = {"error": repr(e)}
     print(json.dumps(line), flush=True)
-    model.close()
     if world > 1:
         dist.destroy_process_group()
 

@@ -46,14 +46,18 @@ extern "C" {
 #define SAGC_ADV_GRPO 0
 #define SAGC_ADV_DAPO 1
 
-#define SAGC_PATH_AUTO 0  /* tcgen05 GEMM while the live batch is large, GEMV in the tail */
+#define SAGC_PATH_AUTO 0  /* tcgen05/TMEM kernels at every batch size when the shapes are multiples of 128 (the
+                             persistent decode-step kernel at <= 64 live rows, per-layer kernels above), else the
+                             register-HMMA kernels: measured faster than the GEMV kernels even with 1 live row */
 #define SAGC_PATH_GEMV 1  /* force the fp32-activation GEMV kernels for every batch size   */
-#define SAGC_PATH_GEMM 2  /* force the tcgen05/TMEM GEMM kernels for every batch size      */
+#define SAGC_PATH_GEMM 2  /* force the tensor-core kernels for every batch size            */
 
 #define SAGC_FLAG_STRUCTURE_ONLY 1  /* run paging / retirement / lengths only, no model forward;
                                        tokens are written as 0 (needs forced_lengths)          */
 #define SAGC_FLAG_LOG            2  /* record the page-allocation and retirement logs          */
 #define SAGC_FLAG_NO_GRAPH       4  /* launch kernels directly instead of through CUDA graphs  */
+#define SAGC_FLAG_TIME_KERNELS   8  /* (implies NO_GRAPH) CUDA events around the three parts of every decode step:
+                                       layer stack, LM head + sampler, advance -> timing->kernel_ms[] */
 
 typedef struct sagc_model sagc_model;
 
@@ -124,6 +128,11 @@ typedef struct {
     double  prefill_flops;
     int64_t total_tokens;       /* generated tokens, all phases + the first token           */
     int64_t kernel_launches;    /* kernels of this library launched by the call             */
+    /* SAGC_FLAG_TIME_KERNELS: device time of the decode steps by part, summed over the rollout:
+       [0] layer stack (the persistent decode-step kernel, or the per-layer kernels), [1] LM head +
+       sampler, [2] advance (retire / compact / page allocation); kernel_steps = steps measured   */
+    double  kernel_ms[3];
+    int64_t kernel_steps;
 } sagc_rollout_timing;
 
 /* Synchronous group rollout (Alg.1 l.7).  sid = p*G + g (prompt-major).
@@ -147,6 +156,17 @@ int sagc_rollout_group_host(sagc_model* m, const int32_t* prompt_tokens, const i
                             int32_t n_prompts, int32_t G, const sagc_rollout_params* params,
                             int32_t* out_tokens, int32_t* out_lengths, float* out_ratio,
                             int32_t* out_len_stats, sagc_rollout_timing* timing, void* stream);
+
+/* Teacher-forced log-prob pass: log pi(y_t | x, y_<t) of every generated token under the same policy
+ * snapshot -- the quantity the GRPO / DAPO loss needs next.  ONE causal pass per sequence over prompt +
+ * completion with the prefill kernels (not token by token), the LM head over every position, log-softmax at the target.
+ *   prompt_tokens dev int32 (concatenated); prompt_offsets HOST int32 [n_prompts+1];
+ *   tokens dev int32 [n_prompts*G][max_new] (as returned by sagc_rollout_group); lengths HOST int32 [n_prompts*G];
+ *   out_logprobs dev float [n_prompts*G][max_new], 0 beyond each length.
+ * Uses (and overwrites) the handle's KV pool and page tables: needs sum(ceil((P + l - 1) / page_tokens)) pages.
+ * Synchronises the stream.  Errors: SAGC_EINVAL, SAGC_EPAGES, SAGC_ECUDA. */
+int sagc_score_tokens(sagc_model* m, const int32_t* prompt_tokens, const int32_t* prompt_offsets, int32_t n_prompts, int32_t G,
+                      const int32_t* tokens, const int32_t* lengths, int32_t max_new, float* out_logprobs, void* stream);
 
 /* Group-relative advantages.  Group g = rewards[off[g] : off[g+1]].
  *   all-equal group (max == min, exact) or size 1: A = 0, keep = 0 (DAPO) / 1 (GRPO)

@@ -122,3 +122,15 @@ def teacher_forced_logits(dec: RefDecoder, prompt: Sequence[int], gen_tokens: Se
     seq = list(int(x) for x in prompt) + [int(x) for x in gen_tokens[: tmax - 1]]
     rows = [P + int(s) - 2 for s in steps]
     return dec.forward_full(seq, logits_at=rows)
+
+
+def token_logprobs(dec: RefDecoder, prompt: Sequence[int], gen_tokens: Sequence[int]) -> np.ndarray:
+    """log pi(y_t | x, y_<t), t = 1..len(gen_tokens): the policy log-probabilities the GRPO / DAPO objective is built
+    from ("compute per-completion rewards" / "form group-relative advantages" act on these
+    sampled completions).  Definition written out: one teacher-forced causal pass, then
+    log-softmax (float64, max-subtracted) of the logits row that predicts token t, read at token t."""
+    L = len(gen_tokens)
+    lg = teacher_forced_logits(dec, prompt, gen_tokens, list(range(1, L + 1))).astype(np.float64)
+    mx = lg.max(axis=1, keepdims=True)
+    lse = mx[:, 0] + np.log(np.exp(lg - mx).sum(axis=1))
+    return lg[np.arange(L), np.asarray(gen_tokens, dtype=np.int64)] - lse

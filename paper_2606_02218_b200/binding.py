@@ -21,10 +21,10 @@ OK, EINVAL, ENOMEM, EPAGES, ECUDA = 0, -1, -2, -3, -4
 MODE_GREEDY, MODE_GUMBEL = 0, 1
 ADV_GRPO, ADV_DAPO = 0, 1
 PATH_AUTO, PATH_GEMV, PATH_GEMM = 0, 1, 2
-FLAG_STRUCTURE_ONLY, FLAG_LOG, FLAG_NO_GRAPH = 1, 2, 4
+FLAG_STRUCTURE_ONLY, FLAG_LOG, FLAG_NO_GRAPH, FLAG_TIME_KERNELS = 1, 2, 4, 8
 
 EXPORTS = [
-    "sagc_model_create", "sagc_model_destroy", "sagc_rollout_group", "sagc_rollout_group_host",
+    "sagc_model_create", "sagc_model_destroy", "sagc_rollout_group", "sagc_rollout_group_host", "sagc_score_tokens",
     "sagc_group_advantage", "sagc_length_stats", "sagc_debug_page_table", "sagc_debug_free_stack",
     "sagc_debug_alloc_log", "sagc_debug_retire_log", "sagc_debug_peak_pages", "sagc_debug_philox",
     "sagc_debug_linear", "sagc_debug_lm_sample", "sagc_debug_attention", "sagc_debug_step_trace", "sagc_last_error", "sagc_version",
@@ -59,7 +59,7 @@ class _Timing(C.Structure):
     _fields_ = [("prefill_ms", C.c_double), ("decode_ms", C.c_double), ("phase_ms", C.c_double * 3),
                 ("phase_steps", C.c_int64 * 3), ("phase_tokens", C.c_int64 * 3), ("phase_bytes", C.c_double * 3),
                 ("prefill_tokens", C.c_int64), ("prefill_flops", C.c_double), ("total_tokens", C.c_int64),
-                ("kernel_launches", C.c_int64)]
+                ("kernel_launches", C.c_int64), ("kernel_ms", C.c_double * 3), ("kernel_steps", C.c_int64)]
 
 
 _lib = None
@@ -82,6 +82,8 @@ def lib():
                 C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(_Timing), C.c_void_p]
         L.sagc_rollout_group.argtypes = roll
         L.sagc_rollout_group_host.argtypes = roll
+        L.sagc_score_tokens.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32,
+                                        C.c_void_p, C.c_void_p]
         L.sagc_group_advantage.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_float,
                                            C.c_void_p, C.c_void_p, C.c_void_p]
         L.sagc_length_stats.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -231,8 +233,22 @@ class Model:
                   "phase_steps": list(tm.phase_steps), "phase_tokens": list(tm.phase_tokens),
                   "phase_bytes": list(tm.phase_bytes), "prefill_tokens": tm.prefill_tokens,
                   "prefill_flops": tm.prefill_flops, "total_tokens": tm.total_tokens,
-                  "kernel_launches": tm.kernel_launches}
+                  "kernel_launches": tm.kernel_launches, "kernel_ms": list(tm.kernel_ms), "kernel_steps": tm.kernel_steps}
         return RolloutOutput(toks, lens, ratio, stats, td, dump_out)
+
+    # -- sagc_score_tokens ---------------------------------------------------------------
+    def score_tokens(self, prompt_tokens, prompt_offsets, G: int, tokens: torch.Tensor, lengths) -> torch.Tensor:
+        """log pi(y_t | x, y_<t) of every generated token: float32 [nseq][max_new] (device), 0 beyond each length."""
+        offs = np.ascontiguousarray(prompt_offsets, dtype=np.int32)
+        n_prompts = offs.shape[0] - 1
+        if not torch.is_tensor(prompt_tokens):
+            prompt_tokens = torch.from_numpy(np.ascontiguousarray(prompt_tokens, dtype=np.int32)).to(self.device)
+        assert tokens.is_cuda and tokens.dtype == torch.int32 and tokens.is_contiguous()
+        lens = np.ascontiguousarray(lengths.cpu().numpy() if torch.is_tensor(lengths) else lengths, dtype=np.int32)
+        out = torch.empty(tokens.shape, dtype=torch.float32, device=self.device)
+        _check(lib().sagc_score_tokens(self._h, prompt_tokens.data_ptr(), offs.ctypes.data, n_prompts, G, tokens.data_ptr(),
+                                       lens.ctypes.data, tokens.shape[1], out.data_ptr(), _stream()))
+        return out
 
     # -- debug / parity exports ---------------------------------------------------------
     def debug_page_table(self) -> np.ndarray:

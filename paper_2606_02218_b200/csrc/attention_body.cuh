@@ -48,6 +48,28 @@ __device__ __forceinline__ void store_out(const AttnArgs& a, int row, int col, f
     }
 }
 
+// element(s) of the activation row that holds q | k | v: fp32, or 64-bit fixed point * 2^-32 * (1/rms of the row)
+static constexpr float ATT_FX_SCALE = 2.3283064365386963e-10f;      // 2^-32
+__device__ __forceinline__ void att_load8(const AttnArgs& a, int row, size_t col, float rs, float (&o)[8]) {
+    if (a.q_fx != nullptr) {
+        const longlong2* p = reinterpret_cast<const longlong2*>(a.q_fx + (size_t)row * a.ldq + col);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const longlong2 v = __ldcg(p + i);
+            o[2 * i] = __ll2float_rn(v.x) * ATT_FX_SCALE * rs;
+            o[2 * i + 1] = __ll2float_rn(v.y) * ATT_FX_SCALE * rs;
+        }
+    } else {
+        const float4 x0 = __ldcg(reinterpret_cast<const float4*>(a.q + (size_t)row * a.ldq + col));
+        const float4 x1 = __ldcg(reinterpret_cast<const float4*>(a.q + (size_t)row * a.ldq + col + 4));
+        o[0] = x0.x; o[1] = x0.y; o[2] = x0.z; o[3] = x0.w; o[4] = x1.x; o[5] = x1.y; o[6] = x1.z; o[7] = x1.w;
+    }
+}
+__device__ __forceinline__ float att_load1(const AttnArgs& a, int row, size_t col, float rs) {
+    if (a.q_fx != nullptr) return __ll2float_rn(__ldcg(a.q_fx + (size_t)row * a.ldq + col)) * ATT_FX_SCALE * rs;
+    return __ldcg(a.q + (size_t)row * a.ldq + col);
+}
+
 __device__ __forceinline__ void ldmatrix_x4_trans(uint32_t (&r)[4], const void* smem_row) {
     const uint32_t a = (uint32_t)__cvta_generic_to_shared(smem_row);
     asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];\n"
@@ -179,27 +201,27 @@ __device__ __forceinline__ void attention_unit(const AttnArgs& a, const int row,
     uint32_t knew = 0, vnew = 0;                    // designated unit: bf16 bits of the new k pair / v element
     {
         const float scale = rsqrtf((float)HD);
-        const float* qp = a.q + (size_t)row * a.ldq + (size_t)(kvh * r + g) * HD + 8 * q;
+        const float rs = a.q_fx != nullptr ? __ldcg(a.q_rstd + row) : 1.f;
+        const size_t qcol = (size_t)(kvh * r + g) * HD + 8 * q;
         float xq[KB][8];
 #pragma unroll
         for (int kb = 0; kb < KB; ++kb) {
-            float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0;
             if (g < r) {
-                x0 = __ldcg(reinterpret_cast<const float4*>(qp + kb * 32));
-                x1 = __ldcg(reinterpret_cast<const float4*>(qp + kb * 32 + 4));
+                att_load8(a, row, qcol + kb * 32, rs, xq[kb]);
+            } else {
+#pragma unroll
+                for (int e = 0; e < 8; ++e) xq[kb][e] = 0.f;
             }
-            xq[kb][0] = x0.x; xq[kb][1] = x0.y; xq[kb][2] = x0.z; xq[kb][3] = x0.w;
-            xq[kb][4] = x1.x; xq[kb][5] = x1.y; xq[kb][6] = x1.z; xq[kb][7] = x1.w;
         }
         if (designated) {
             // raw k (pair i, i + hd/2) and v of the newest position from the same qkv row
-            const float* kp = a.q + (size_t)row * a.ldq + (size_t)a.Hq * HD + (size_t)kvh * HD;
-            const float* vp = kp + (size_t)a.Hkv * HD;
+            const size_t kcol = (size_t)a.Hq * HD + (size_t)kvh * HD;
+            const size_t vcol = kcol + (size_t)a.Hkv * HD;
             if (tid < HD / 2) {
-                const float k0 = __ldcg(kp + tid), k1 = __ldcg(kp + tid + HD / 2);
+                const float k0 = att_load1(a, row, kcol + tid, rs), k1 = att_load1(a, row, kcol + tid + HD / 2, rs);
                 knew = f32_to_bf16_bits(k0 * kcs.x - k1 * kcs.y) | (f32_to_bf16_bits(k1 * kcs.x + k0 * kcs.y) << 16);
             }
-            if (tid < HD) vnew = f32_to_bf16_bits(__ldcg(vp + tid));
+            if (tid < HD) vnew = f32_to_bf16_bits(att_load1(a, row, vcol + tid, rs));
         }
         if (fuse) {
 #pragma unroll

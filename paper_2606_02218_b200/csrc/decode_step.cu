@@ -1,24 +1,27 @@
 // decode_step.cu -- ONE persistent kernel for the whole layer stack of a decode step (steps a5-a10 of
 // DESIGN.md; <= 64 live rows): embedding + per layer { QKV | RoPE + KV append + paged attention | O + residual |
-// gate/up + SwiGLU | down + residual }.  One CTA per SM; kernel boundaries are replaced by grid-wide
-// arrive/poll counters in L2, and -- the point of the exercise -- the weight stream never stops at them:
+// gate/up + SwiGLU | down + residual } + the operand of the LM head.  One CTA per SM; kernel boundaries are
+// replaced by grid-wide arrive/poll counters in L2, and -- the point of the exercise -- the weight stream never
+// stops at them:
 //
 //   warp 0   A producer : walks this CTA's static work list (every layer, every GEMM phase) and TMA-loads the
 //                         128 x 64 bf16 weight tiles into a ring of 16 KB slots.  Weights depend on nothing,
 //                         so it runs as far ahead as the ring allows, across phase and layer boundaries.
-//   warp 1   B producer : loads the activation operand (pre-split hi/lo bf16 rows) of the
-//                         same work list into its own ring slots as soon as the phase that produces it has
-//                         completed on every CTA.
-//   warp 2   MMA issuer : tcgen05.mma (weights = A, M = 128; activations = B, N = 2 x batch), fp32 in TMEM.
-//   warp 3   owns the TMEM allocation.
-//   warps 4-11 workers  : epilogues (TMEM -> registers -> fused residual / SwiGLU / next-norm -> L2), the
-//                         split-K reduction, the attention units (attention_body.cuh) and the embedding rows.
+//   warp 1   MMA issuer : tcgen05.mma (weights = A, M = 128; activations = B, N = 2 x batch), fp32 in TMEM.
+//   warp 2   owns the TMEM allocation; warp 3 idle.
+//   warps 4-11 workers  : build the activation operand of their unit in shared memory (hi/lo bf16 split, 128-byte
+//                         swizzle, RMSNorm gain / SwiGLU fused), drain the accumulators, run the attention units
+//                         (attention_body.cuh), the per-row bookkeeping (residual stream, 1/rms) and the embedding.
 //
-// Work decomposition (host, build_step_plan): a GEMM phase is cut into units (128-row weight tile, k range);
-// unit -> CTA is static.  K is split so that every SM streams a share of every matrix.  The KS partial tiles
-// of an output tile go through an L2 scratch; a per-tile counter tells the KS contributors when all partials
-// have landed, and contributor `rank` then finishes batch rows rank, rank + KS, ... (sum in rank order:
-// deterministic).  All counters are double-buffered by step parity: step t uses set t & 1 and clears the other.
+// Data flow between phases (what makes a phase boundary ONE L2 round trip): a GEMM phase never stores finished
+// activations.  Every unit (128-row weight tile x k range; K is split so that every SM streams a share of every
+// matrix) adds its partial products to a 64-bit FIXED-POINT accumulator in L2 (value * 2^32, red.add.u64: integer
+// addition is associative, so the sum is bit-reproducible whatever the arrival order).  The consumer of the next
+// phase reads the finished sums of exactly the k columns its own unit needs, applies what sits between the two GEMMs
+// (residual + norm gain, or SwiGLU) and writes the hi/lo bf16 operand tile straight into its shared memory.
+// 1/rms is a per-row scalar: it is computed on the side by the CTA that owns the row (which also carries the fp32
+// residual stream forward) and applied one phase later (attention scales q, k, v; the down projection scales gate
+// and up), so it is never on the critical path.
 #include <cuda.h>
 
 #include <algorithm>
@@ -34,25 +37,31 @@ namespace sagc {
 
 static constexpr int STEP_THREADS = 384;
 static constexpr int STEP_SLOT = 16384;                  // ring slot: one 128 x 64 bf16 weight tile
-static constexpr int STEP_ATT_BYTES = 65536;             // K/V staging of the attention units
-static constexpr int STEP_MISC = 3072;                   // barriers, plan copy, rstd / ssq scratch
-static constexpr int STEP_SCR_SLOT = 2 * 64 * 128;       // floats per split-K scratch slot: [na][m][row]
+static constexpr int STEP_ATT_BYTES = 65536;             // K/V staging of the attention units; GEMM phases: 2 x 32 KB B buffers
+static constexpr int STEP_BBUF = 32768;
+static constexpr int STEP_MISC = 3072;                   // barriers, plan copy, small scratch
 static constexpr unsigned long long STEP_WATCHDOG_NS = 4000000000ull;
+static constexpr float FX_SCALE = 4294967296.f;          // 2^32
+static constexpr float FX_INV = 2.3283064365386963e-10f; // 2^-32
 
 // attention geometry inside the step kernel: 64 KB of K/V staging either way
-template <int HD> struct StepAtt { static constexpr int WARPS = HD >= 128 ? 4 : 8; static constexpr int NSTAGE = 2; };
+template <int HD> struct StepAtt { static constexpr int WARPS = 4; static constexpr int NSTAGE = HD >= 128 ? 2 : 4; };   // 64-token tiles
 
 struct StepDev {
-    int n_layers, n_cta, NB, n_slots, bper;
+    int n_layers, n_cta, NB, n_slots, chunk;             // chunk = k blocks per B buffer = STEP_BBUF / (NB * 128)
+    int prefetch;                        // k blocks the L2 prefetch runs ahead of the ring loads inside a unit (0 = off)
     StepGemm g[4];
     const CUtensorMap* wmaps;            // device [n_layers][7]: q k v o g u d (box 64 x 128)
     const StepPhasePlan* plan;           // device [4][n_cta]
-    float* x; float* qkv; bf16_t* xs; bf16_t* att_s; bf16_t* act_s; float* ssq;
+    float* xa; float* xb;                // fp32 residual stream, ping-pong [64][d_model]
+    long long* accQ; long long* accO; long long* accG; long long* accD;     // fixed-point sums [64][Nqkv | d | 2 d_ff | d]
+    float* rstd1; float* rstd2;          // [64] 1/rms of the rows entering QKV / gate-up
+    float* x; bf16_t* xs; float* ssq;    // LM-head operand (final residual rows, pre-split x * w_final, sums of squares)
+    bf16_t* att_s;
     int ssq_ld, d_tiles, d_model, Nqkv, qd, d_ff;
     const bf16_t* const* norm1; const bf16_t* const* norm2; const bf16_t* final_norm; const bf16_t* embed;
     float eps;
-    float* scratch;
-    unsigned* sync_base; int gbar_n, tcnt_n, tiles_per_layer;        // [2][gbar_n + tcnt_n]
+    unsigned* sync_base; int gbar_n;     // [2][gbar_n] phase counters, double-buffered by step parity
     const int* live; const int* pos; const int* ctx; const int* tok; const int* n_live; const int* step; int m_max;
     AttnArgs att; bf16_t* kv_pool; size_t layer_stride;
     int* err;
@@ -68,6 +77,11 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
 __device__ __forceinline__ void red_release_add(unsigned* p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;\n" ::"l"(p), "r"(v) : "memory");
 }
+__device__ __forceinline__ void red_add_fx(long long* p, float v) {
+    const long long q = __float2ll_rn(v * FX_SCALE);
+    asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;\n" ::"l"(p), "l"(q) : "memory");
+}
+__device__ __forceinline__ float fx_to_f32(long long v) { return __ll2float_rn(v) * FX_INV; }
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;\n" : "=l"(t));
@@ -86,22 +100,7 @@ __device__ __forceinline__ void step_wait_mbar(uint64_t* bar, uint32_t parity, i
     while (!mbar_try(bar, parity))
         if (((++n) & 255u) == 0 && globaltimer_ns() - t0 > STEP_WATCHDOG_NS) step_die(err, code);
 }
-__device__ __forceinline__ unsigned ld_relaxed_u32(const unsigned* p) {
-    unsigned v;
-    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void step_wait_count(const unsigned* ctr, unsigned target, int* err, int code, bool relaxed = false) {
-    if (relaxed) {      // poll with relaxed loads, one acquire fence at the end
-        if (ld_relaxed_u32(ctr) < target) {
-            const unsigned long long t0 = globaltimer_ns();
-            unsigned n = 0;
-            while (ld_relaxed_u32(ctr) < target)
-                if (((++n) & 1023u) == 0 && globaltimer_ns() - t0 > STEP_WATCHDOG_NS) step_die(err, code);
-        }
-        asm volatile("fence.acq_rel.gpu;\n" ::: "memory");
-        return;
-    }
+__device__ __forceinline__ void step_wait_count(const unsigned* ctr, unsigned target, int* err, int code) {
     if (ld_acquire_u32(ctr) >= target) return;
     const unsigned long long t0 = globaltimer_ns();
     unsigned n = 0;
@@ -121,13 +120,12 @@ __device__ __forceinline__ void worker_sync() { asm volatile("bar.sync 1, 256;\n
 __device__ __forceinline__ float silu_f(float z) { return z / (1.f + __expf(-z)); }
 
 struct StepShared {                      // lives in the STEP_MISC region
-    uint64_t full[12], empty[12], acc_full[2];
+    uint64_t full[12], empty[12], acc_full[2], bfull[2], bempty[2];
     uint32_t tmem_slot; int M, par, ns, pad;
     StepPhasePlan pl[4];
-    float rstd[64];
-    float ssq_s[4][64];
     float red[8];
     int ctx_max[8];
+    float rstd[64];
 };
 static_assert(sizeof(StepShared) <= STEP_MISC, "StepShared outgrew its region");
 
@@ -146,26 +144,54 @@ __device__ __forceinline__ const CUtensorMap* step_wmap(const StepDev& a, const 
     return &w7[6];
 }
 
+// 8 consecutive k of batch row m -> rows 2m (hi) and 2m+1 (lo) of a K-major, 128-byte-swizzled B tile of one k block
+// (tile = NB rows x 128 B; 16-byte chunk c of row r sits at chunk c ^ (r & 7))
+__device__ __forceinline__ void store_b_chunk(uint8_t* tile, int m, int c, const float (&v)[8]) {
+    uint32_t hi[4], lo[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) split2(v[2 * i], v[2 * i + 1], hi[i], lo[i]);
+    const int r0 = 2 * m, r1 = 2 * m + 1;
+    *reinterpret_cast<uint4*>(tile + (size_t)r0 * 128 + ((c ^ (r0 & 7)) << 4)) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+    *reinterpret_cast<uint4*>(tile + (size_t)r1 * 128 + ((c ^ (r1 & 7)) << 4)) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+}
+__device__ __forceinline__ void load_fx8(const long long* p, float (&o)[8]) {
+    const longlong2* q = reinterpret_cast<const longlong2*>(p);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const longlong2 v = __ldcg(q + i);
+        o[2 * i] = fx_to_f32(v.x);
+        o[2 * i + 1] = fx_to_f32(v.y);
+    }
+}
+__device__ __forceinline__ void load_f8(const float* p, float (&o)[8]) {
+    const float4 a = __ldcg(reinterpret_cast<const float4*>(p)), b = __ldcg(reinterpret_cast<const float4*>(p + 4));
+    o[0] = a.x; o[1] = a.y; o[2] = a.z; o[3] = a.w; o[4] = b.x; o[5] = b.y; o[6] = b.z; o[7] = b.w;
+}
+__device__ __forceinline__ void load_bf8(const bf16_t* p, float (&o)[8]) {
+    const uint4 w = *reinterpret_cast<const uint4*>(p);
+    o[0] = bf16lo_to_f32(w.x); o[1] = bf16hi_to_f32(w.x); o[2] = bf16lo_to_f32(w.y); o[3] = bf16hi_to_f32(w.y);
+    o[4] = bf16lo_to_f32(w.z); o[5] = bf16hi_to_f32(w.z); o[6] = bf16lo_to_f32(w.w); o[7] = bf16hi_to_f32(w.w);
+}
+
 template <int HD>
 __global__ void __launch_bounds__(STEP_THREADS, 1)
-k_decode_step(const __grid_constant__ CUtensorMap tmXs, const __grid_constant__ CUtensorMap tmAtt,
-              const __grid_constant__ CUtensorMap tmAct, const StepDev a) {
+k_decode_step(const StepDev a) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     uint8_t* ring = smem;
-    uint8_t* att_kv = smem + (size_t)a.n_slots * STEP_SLOT;
+    uint8_t* att_kv = smem + (size_t)a.n_slots * STEP_SLOT;          // attention K/V ring | the two B buffers of the GEMM phases
     AttSmall* att_sm = reinterpret_cast<AttSmall*>(att_kv + STEP_ATT_BYTES);
     StepShared* sh = reinterpret_cast<StepShared*>(reinterpret_cast<uint8_t*>(att_sm) + ((sizeof(AttSmall) + 15) & ~(size_t)15));
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int cta = blockIdx.x, nCTA = a.n_cta, NS = a.n_slots, NB = a.NB, L = a.n_layers;
+    const int cta = blockIdx.x, nCTA = a.n_cta, NS = a.n_slots, NB = a.NB, L = a.n_layers, CH = a.chunk;
 
     if (tid < 4) sh->pl[tid] = a.plan[(size_t)tid * nCTA + cta];
-    if (warp == 2 && lane == 0) {
+    if (warp == 1 && lane == 0) {
         for (int s = 0; s < NS; ++s) { mbar_init(&sh->full[s], 1); mbar_init(&sh->empty[s], 1); }
-        mbar_init(&sh->acc_full[0], 1); mbar_init(&sh->acc_full[1], 1);
+        for (int s = 0; s < 2; ++s) { mbar_init(&sh->acc_full[s], 1); mbar_init(&sh->bfull[s], 1); mbar_init(&sh->bempty[s], 1); }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
-    if (warp == 3) {
+    if (warp == 2) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&sh->tmem_slot)), "n"(512));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n");
     }
@@ -178,11 +204,14 @@ k_decode_step(const __grid_constant__ CUtensorMap tmXs, const __grid_constant__ 
 
     if (warp == 0) {
         // =========================== A producer: weights, as far ahead as the ring allows ===========================
+        // Besides filling the ring, the producer asks the TMA unit to pull the tile `a.prefetch` k blocks further along
+        // the same unit into L2: while the consumers sit in a phase boundary the ring is full, but HBM keeps streaming.
         if (lane == 0) {
             unsigned n = 0;
+            for (int i = 0; i < 7 && L > 0; ++i) tma_prefetch_desc(&a.wmaps[i]);
             for (int l = 0; l < L; ++l) {
                 const CUtensorMap* w7 = a.wmaps + (size_t)l * 7;
-                for (int i = 0; i < 7; ++i) tma_prefetch_desc(&w7[i]);
+                if (l + 1 < L) for (int i = 0; i < 7; ++i) tma_prefetch_desc(&w7[7 + i]);
                 for (int ph = 0; ph < 4; ++ph) {
                     const int NA = a.g[ph].na;
                     for (int s = 0; s < sh->pl[ph].nseg; ++s) {
@@ -190,92 +219,51 @@ k_decode_step(const __grid_constant__ CUtensorMap tmXs, const __grid_constant__ 
                         int arow;
                         const CUtensorMap* m0 = step_wmap(a, w7, ph, sg.tile, 0, arow);
                         const CUtensorMap* m1 = step_wmap(a, w7, ph, sg.tile, 1, arow);
-                        for (int kbg = sg.kb0; kbg < sg.kb1; kbg += a.bper) {
-                            const int nbk = min(a.bper, sg.kb1 - kbg);
-                            ++n;                                             // the group's B slot (filled by warp 1)
-                            for (int j = 0; j < nbk; ++j)
-                                for (int na = 0; na < NA; ++na, ++n) {
-                                    const unsigned slot = n % NS, use = n / NS;
-                                    if (use > 0) step_wait_mbar(&sh->empty[slot], (use - 1) & 1, a.err, 1);
-                                    mbar_expect_tx(&sh->full[slot], STEP_SLOT);
-                                    tma_load_2d(ring + (size_t)slot * STEP_SLOT, na ? m1 : m0, &sh->full[slot], (kbg + j) * 64, arow);
-                                }
-                        }
+                        for (int kb = sg.kb0; kb < sg.kb1; ++kb)
+                            for (int na = 0; na < NA; ++na, ++n) {
+                                const unsigned slot = n % NS, use = n / NS;
+                                if (a.prefetch > 0 && kb + a.prefetch < sg.kb1)
+                                    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];\n" ::"l"(na ? m1 : m0),
+                                                 "r"((kb + a.prefetch) * 64), "r"(arow) : "memory");
+                                if (use > 0) step_wait_mbar(&sh->empty[slot], (use - 1) & 1, a.err, 1);
+                                mbar_expect_tx(&sh->full[slot], STEP_SLOT);
+                                tma_load_2d(ring + (size_t)slot * STEP_SLOT, na ? m1 : m0, &sh->full[slot], kb * 64, arow);
+                            }
                     }
                 }
             }
         }
         __syncwarp();
     } else if (warp == 1) {
-        // =========================== B producer: activations, gated by the producing phase ===========================
-        if (lane == 0) {
-            pdl_wait();
-            const int par = *a.step & 1;
-            const bool tron = tr_cta && (unsigned long long)*a.step == a.trace[0];
-            const unsigned* gbar = a.sync_base + (size_t)par * (a.gbar_n + a.tcnt_n);
-            tma_prefetch_desc(&tmXs); tma_prefetch_desc(&tmAtt); tma_prefetch_desc(&tmAct);
-            unsigned n = 0;
-            for (int l = 0; l < L; ++l) {
-                for (int ph = 0; ph < 4; ++ph) {
-                    const int NA = a.g[ph].na;
-                    const int p = 1 + l * 5 + (ph == 0 ? 0 : ph + 1);            // phase index of this GEMM
-                    const CUtensorMap* bm = (ph == 1) ? &tmAtt : (ph == 3 ? &tmAct : &tmXs);
-                    bool opened = false;
-                    for (int s = 0; s < sh->pl[ph].nseg; ++s) {
-                        const StepSeg sg = sh->pl[ph].seg[s];
-                        for (int kbg = sg.kb0; kbg < sg.kb1; kbg += a.bper) {
-                            const int nbk = min(a.bper, sg.kb1 - kbg);
-                            const unsigned slot = n % NS, use = n / NS;
-                            if (!opened) {
-                                step_wait_count(gbar + (p - 1), (unsigned)nCTA, a.err, 2, (a.flags & 4) != 0);
-                                asm volatile("fence.proxy.async;\n" ::: "memory");   // generic-proxy writes of other SMs -> TMA reads
-                                opened = true;
-                                step_trace(a, tron, 1, 0, p);
-                            }
-                            if (use > 0) step_wait_mbar(&sh->empty[slot], (use - 1) & 1, a.err, 3);
-                            mbar_expect_tx(&sh->full[slot], (uint32_t)(nbk * NB * 128));
-                            for (int j = 0; j < nbk; ++j)
-                                tma_load_2d(ring + (size_t)slot * STEP_SLOT + (size_t)j * NB * 128, bm, &sh->full[slot], (kbg + j) * 64, 0);
-                            n += 1 + nbk * NA;
-                        }
-                    }
-                }
-            }
-        }
-        __syncwarp();
-    } else if (warp == 2) {
         // =========================== MMA issuer ===========================
         if (lane == 0) {
             const uint32_t idesc = umma_idesc(NB);
-            unsigned n = 0;
+            unsigned n = 0, cn = 0;                       // ring item / B chunk sequence numbers
             for (int l = 0; l < L; ++l) {
                 for (int ph = 0; ph < 4; ++ph) {
                     const int NA = a.g[ph].na;
                     for (int s = 0; s < sh->pl[ph].nseg; ++s) {
                         const StepSeg sg = sh->pl[ph].seg[s];
-                        for (int kbg = sg.kb0; kbg < sg.kb1; kbg += a.bper) {
-                            const int nbk = min(a.bper, sg.kb1 - kbg);
-                            const unsigned bslot = n % NS, buse = n / NS;
-                            ++n;
-                            step_wait_mbar(&sh->full[bslot], buse & 1, a.err, 4);
-                            if (kbg == sg.kb0) step_trace(a, tr_cta, 2, 0, 1 + l * 5 + (ph == 0 ? 0 : ph + 1));
-                            for (int j = 0; j < nbk; ++j)
+                        for (int kc = sg.kb0; kc < sg.kb1; kc += CH, ++cn) {
+                            const int nk = min(CH, sg.kb1 - kc);
+                            const unsigned buf = cn & 1u, buse = cn >> 1;
+                            step_wait_mbar(&sh->bfull[buf], buse & 1, a.err, 4);
+                            for (int j = 0; j < nk; ++j)
                                 for (int na = 0; na < NA; ++na, ++n) {
                                     const unsigned slot = n % NS, use = n / NS;
                                     step_wait_mbar(&sh->full[slot], use & 1, a.err, 5);
                                     tc_fence_after();
                                     const uint64_t adesc = umma_desc_sw128(smem_u32(ring + (size_t)slot * STEP_SLOT));
-                                    const uint64_t bdesc = umma_desc_sw128(smem_u32(ring + (size_t)bslot * STEP_SLOT + (size_t)j * NB * 128));
+                                    const uint64_t bdesc = umma_desc_sw128(smem_u32(att_kv + (size_t)buf * STEP_BBUF + (size_t)j * NB * 128));
                                     const uint32_t dcol = tmem_base + (uint32_t)((s * 2 + na) * NB);
 #pragma unroll
                                     for (int k = 0; k < 4; ++k)
-                                        tc_mma(dcol, adesc + 2 * k, bdesc + 2 * k, idesc, (kbg + j > sg.kb0 || k > 0) ? 1u : 0u);
+                                        tc_mma(dcol, adesc + 2 * k, bdesc + 2 * k, idesc, (kc + j > sg.kb0 || k > 0) ? 1u : 0u);
                                     tc_commit(&sh->empty[slot]);
                                 }
-                            tc_commit(&sh->empty[bslot]);
+                            tc_commit(&sh->bempty[buf]);
                         }
                         tc_commit(&sh->acc_full[s]);
-                        step_trace(a, tr_cta, 2, 1, 1 + l * 5 + (ph == 0 ? 0 : ph + 1));
                     }
                 }
             }
@@ -285,6 +273,7 @@ k_decode_step(const __grid_constant__ CUtensorMap tmXs, const __grid_constant__ 
         // =========================== workers ===========================
         const int wt = tid - 128, wi = warp - 4, lg = wi & 3, h = wi >> 2;
         const int row = lg * 32 + lane;                       // output feature inside a 128-row tile = TMEM lane
+        const int d = a.d_model, F = a.d_ff;
         pdl_wait();
         if (wt == 0) {
             sh->M = min(*a.n_live, a.m_max);
@@ -294,11 +283,10 @@ k_decode_step(const __grid_constant__ CUtensorMap tmXs, const __grid_constant__ 
         const int M = sh->M, par = sh->par;
         const bool tron = tr_cta && wt == 0 && (unsigned long long)*a.step == a.trace[0];
         step_trace(a, tron, 3, 9, 0);
-        unsigned* gbar = a.sync_base + (size_t)par * (a.gbar_n + a.tcnt_n);
-        unsigned* tcnt = gbar + a.gbar_n;
+        unsigned* gbar = a.sync_base + (size_t)par * a.gbar_n;
         {   // clear the other parity set for the next step (nobody touches it during this one)
-            unsigned* other = a.sync_base + (size_t)(par ^ 1) * (a.gbar_n + a.tcnt_n);
-            for (int i = cta * 256 + wt; i < a.gbar_n + a.tcnt_n; i += nCTA * 256) other[i] = 0u;
+            unsigned* other = a.sync_base + (size_t)(par ^ 1) * a.gbar_n;
+            for (int i = cta * 256 + wt; i < a.gbar_n; i += nCTA * 256) other[i] = 0u;
         }
         // largest context of the step -> number of attention K-splits (same value on every CTA)
         {
@@ -314,7 +302,7 @@ k_decode_step(const __grid_constant__ CUtensorMap tmXs, const __grid_constant__ 
                 constexpr int TILE = StepAtt<HD>::WARPS * 16;
                 const int units0 = max(1, M * a.att.Hkv);
                 int ns = nCTA / units0;
-                const int cap = c2 / (2 * TILE);
+                const int cap = (c2 + TILE - 1) / TILE;          // at least one tile per split
                 if (ns > cap) ns = cap;
                 if (ns > 32) ns = 32;
                 if (ns < 1) ns = 1;
@@ -324,78 +312,71 @@ k_decode_step(const __grid_constant__ CUtensorMap tmXs, const __grid_constant__ 
         }
         const int ns_att = sh->ns;
         auto arrive = [&](int p) {
-            if (!(a.flags & 2)) asm volatile("fence.proxy.async;\n" ::: "memory");     // this thread's global writes -> later TMA reads elsewhere
-            if (!(a.flags & 1)) __threadfence();
-            worker_sync();
-            if (wt == 0) red_release_add(gbar + p, 1u);
+            worker_sync();                                    // every worker's stores / reds of this phase are issued ...
+            if (wt == 0) red_release_add(gbar + p, 1u);       // ... and ordered before this release (cumulative over the barrier)
             step_trace(a, tron, 3, 8, p);
         };
         auto wait_phase = [&](int p) {
-            if (wt == 0) step_wait_count(gbar + p, (unsigned)nCTA, a.err, 6, (a.flags & 4) != 0);
+            if (wt == 0) step_wait_count(gbar + p, (unsigned)nCTA, a.err, 6);
             worker_sync();
             step_trace(a, tron, 3, 0, p + 1);
         };
-
-        // ---- phase 0: embedding rows (x, pre-split x * w_norm1[0], sum of squares) ----
-        for (int r0 = cta; r0 < M; r0 += nCTA) {
-            const int d = a.d_model;
-            const bf16_t* src = a.embed + (size_t)a.tok[r0] * d;
-            const bf16_t* nw = a.norm1[0];
-            float acc = 0.f;
-            for (int k = wt; k < d; k += 256) {
-                const float v = bf16_to_f32(src[k]);
-                a.x[(size_t)r0 * d + k] = v;
-                acc += v * v;
-                const float xw = v * bf16_to_f32(nw[k]);
-                const uint32_t hi = f32_to_bf16_bits(xw);
-                a.xs[(size_t)(2 * r0) * d + k] = (bf16_t)hi;
-                a.xs[(size_t)(2 * r0 + 1) * d + k] = (bf16_t)f32_to_bf16_bits(xw - __uint_as_float(hi << 16));
+        // zero rows [0, M) of a fixed-point accumulator (all CTAs share the work)
+        auto zero_acc = [&](long long* acc, int ncol) {
+            const int n2 = M * (ncol / 2);
+            longlong2* p2 = reinterpret_cast<longlong2*>(acc);
+            for (int i = cta * 256 + wt; i < n2; i += nCTA * 256) p2[i] = make_longlong2(0ll, 0ll);
+        };
+        // the CTA that owns row m (cta == m) carries the fp32 residual stream forward: xout[m] = xin[m] + acc[m],
+        // and publishes 1/rms of the new row
+        auto own_row = [&](const float* xin, const long long* acc, float* xout, float* rstd_out) {
+            if (cta >= M) return;
+            const int m = cta;
+            float ss = 0.f;
+            for (int k = wt * 4; k < d; k += 1024) {
+                const float4 xv = __ldcg(reinterpret_cast<const float4*>(xin + (size_t)m * d + k));
+                const longlong2 a0 = __ldcg(reinterpret_cast<const longlong2*>(acc + (size_t)m * d + k));
+                const longlong2 a1 = __ldcg(reinterpret_cast<const longlong2*>(acc + (size_t)m * d + k + 2));
+                float4 o;
+                o.x = xv.x + fx_to_f32(a0.x); o.y = xv.y + fx_to_f32(a0.y); o.z = xv.z + fx_to_f32(a1.x); o.w = xv.w + fx_to_f32(a1.y);
+                *reinterpret_cast<float4*>(xout + (size_t)m * d + k) = o;
+                ss += o.x * o.x + o.y * o.y + o.z * o.z + o.w * o.w;
             }
-            acc = warp_sum(acc);
-            if (lane == 0) sh->red[wi] = acc;
+            ss = warp_sum(ss);
+            if (lane == 0) sh->red[wi] = ss;
             worker_sync();
             if (wt == 0) {
                 float t = 0.f;
                 for (int i = 0; i < 8; ++i) t += sh->red[i];
-                a.ssq[r0] = t;
-                for (int i = 1; i < a.d_tiles; ++i) a.ssq[(size_t)i * a.ssq_ld + r0] = 0.f;
+                rstd_out[m] = rsqrtf(t / (float)d + a.eps);
             }
             worker_sync();
+        };
+
+        // ---- phase 0: embedding rows -> xa; every accumulator starts the step at zero ----
+        if (cta < M) {
+            const bf16_t* src = a.embed + (size_t)a.tok[cta] * d;
+            for (int k = wt * 8; k < d; k += 2048) {
+                float v[8];
+                load_bf8(src + k, v);
+                *reinterpret_cast<float4*>(a.xa + (size_t)cta * d + k) = make_float4(v[0], v[1], v[2], v[3]);
+                *reinterpret_cast<float4*>(a.xa + (size_t)cta * d + k + 4) = make_float4(v[4], v[5], v[6], v[7]);
+            }
         }
+        zero_acc(a.accQ, a.Nqkv); zero_acc(a.accO, d); zero_acc(a.accG, 2 * F); zero_acc(a.accD, d);
         arrive(0);
 
         unsigned acc_use[2] = {0u, 0u};
-        // final epilogue of one output element group: thread = feature n of `tile`, batch row m
-        auto finish = [&](int ph, int l, int tile, int m, float acc0, float acc1, float res, float nw) {
-            const int n = tile * 128 + row;
-            if (ph == 0) {
-                a.qkv[(size_t)m * a.Nqkv + n] = acc0 * sh->rstd[m];
-            } else if (ph == 2) {
-                const float sc = sh->rstd[m];
-                const float o = silu_f(acc0 * sc) * (acc1 * sc);
-                const uint32_t hi = f32_to_bf16_bits(o);
-                a.act_s[(size_t)(2 * m) * a.d_ff + n] = (bf16_t)hi;
-                a.act_s[(size_t)(2 * m + 1) * a.d_ff + n] = (bf16_t)f32_to_bf16_bits(o - __uint_as_float(hi << 16));
-            } else {
-                const float o = res + acc0;
-                a.x[(size_t)m * a.d_model + n] = o;
-                const float xw = o * nw;
-                const uint32_t hi = f32_to_bf16_bits(xw);
-                a.xs[(size_t)(2 * m) * a.d_model + n] = (bf16_t)hi;
-                a.xs[(size_t)(2 * m + 1) * a.d_model + n] = (bf16_t)f32_to_bf16_bits(xw - __uint_as_float(hi << 16));
-                const float q2 = warp_sum(o * o);
-                if (lane == 0) sh->ssq_s[lg][m] = q2;
-            }
-        };
-
+        unsigned cn = 0;                                      // B chunk sequence number (same walk as the MMA issuer)
         for (int l = 0; l < L; ++l) {
             for (int phx = 0; phx < 5; ++phx) {
                 const int p = 1 + l * 5 + phx;
+                wait_phase(p - 1);
                 if (phx == 1) {
-                    // ---------------- attention (fused RoPE + KV append) ----------------
+                    // ---------------- attention (fused RoPE + KV append); accD is free again ----------------
+                    zero_acc(a.accD, d);
                     const int units = M * a.att.Hkv * ns_att;
                     if (cta < units) {
-                        wait_phase(p - 1);
                         AttnArgs aa = a.att;
                         aa.kv_layer = a.kv_pool + (size_t)l * a.layer_stride;
                         aa.kv_layer_w = a.kv_pool + (size_t)l * a.layer_stride;
@@ -410,112 +391,155 @@ k_decode_step(const __grid_constant__ CUtensorMap tmXs, const __grid_constant__ 
                 }
                 const int ph = phx == 0 ? 0 : phx - 1;               // 0 QKV, 1 O, 2 gate/up, 3 down
                 const int nseg = sh->pl[ph].nseg;
-                if (nseg > 0) {
-                    const int NA = a.g[ph].na;
-                    const bool resid = (ph == 1 || ph == 3);
-                    wait_phase(p - 1);
-                    if (ph == 0 || ph == 2) {                         // fused RMSNorm of the input: 1/rms from the partial sums of squares
-                        if (wt < M) {
-                            float t = 0.f;
-                            for (int i = 0; i < a.d_tiles; ++i) t += __ldcg(a.ssq + (size_t)i * a.ssq_ld + wt);
-                            sh->rstd[wt] = rsqrtf(t / (float)a.d_model + a.eps);
-                        }
-                        worker_sync();
-                    }
-                    const bf16_t* nwp = nullptr;
-                    if (ph == 1) nwp = a.norm2[l];
-                    if (ph == 3) nwp = (l + 1 < L) ? a.norm1[l + 1] : a.final_norm;
-                    bool any_split = false;
-                    for (int s = 0; s < nseg; ++s) {
-                        const StepSeg sg = sh->pl[ph].seg[s];
-                        const int n = sg.tile * 128 + row;
-                        const float nw = resid ? bf16_to_f32(nwp[n]) : 1.f;
-                        step_wait_mbar(&sh->acc_full[s], acc_use[s] & 1, a.err, 7);
-                        ++acc_use[s];
-                        tc_fence_after();
-                        step_trace(a, tron, 3, 1, p);
-                        if (sg.ks == 1) {
-                            for (int c = h; c * 16 < M && c < NB / 32; c += 2) {
-                                float res[16];
-#pragma unroll
-                                for (int j = 0; j < 16; ++j)
-                                    res[j] = (resid && c * 16 + j < M) ? __ldcg(a.x + (size_t)(c * 16 + j) * a.d_model + n) : 0.f;
-                                float v0[32], v1[32];
-                                tc_ld32(tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)((s * 2) * NB + c * 32), v0);
-                                if (NA == 2) tc_ld32(tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)((s * 2 + 1) * NB + c * 32), v1);
-#pragma unroll
-                                for (int j = 0; j < 16; ++j) {
-                                    const int m = c * 16 + j;
-                                    if (m < M) finish(ph, l, sg.tile, m, v0[2 * j] + v0[2 * j + 1], NA == 2 ? v1[2 * j] + v1[2 * j + 1] : 0.f, res[j], nw);
-                                }
-                            }
-                        } else {
-                            any_split = true;
-                            float* mine = a.scratch + (size_t)(sg.slot0 + sg.rank) * STEP_SCR_SLOT;
-                            for (int na = 0; na < NA; ++na)
-                                for (int c = h; c * 16 < M && c < NB / 32; c += 2) {
-                                    float v[32];
-                                    tc_ld32(tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)((s * 2 + na) * NB + c * 32), v);
-#pragma unroll
-                                    for (int j = 0; j < 16; ++j)
-                                        if (c * 16 + j < M) __stcg(mine + ((size_t)na * 64 + c * 16 + j) * 128 + row, v[2 * j] + v[2 * j + 1]);
-                                }
-                        }
-                        if (sg.ks == 1 && resid) {                    // partial sums of squares of the new residual rows of this tile
-                            worker_sync();
-                            if (wt < M)
-                                a.ssq[(size_t)sg.tile * a.ssq_ld + wt] = sh->ssq_s[0][wt] + sh->ssq_s[1][wt] + sh->ssq_s[2][wt] + sh->ssq_s[3][wt];
-                            worker_sync();
-                        }
-                    }
-                    step_trace(a, tron, 3, 2, p);
-                    if (any_split) {
-                        unsigned* tc = tcnt + (size_t)l * a.tiles_per_layer + a.g[ph].tile_ctr_off;
-                        if (!(a.flags & 8)) __threadfence();
-                        worker_sync();
-                        if (wt == 0)
-                            for (int s = 0; s < nseg; ++s)
-                                if (sh->pl[ph].seg[s].ks > 1) red_release_add(tc + sh->pl[ph].seg[s].tile, 1u);
-                        for (int s = 0; s < nseg; ++s) {
-                            const StepSeg sg = sh->pl[ph].seg[s];
-                            if (sg.ks == 1) continue;
-                            if (wt == 0) step_wait_count(tc + sg.tile, (unsigned)sg.ks, a.err, 8, (a.flags & 4) != 0);
-                            worker_sync();
-                            step_trace(a, tron, 3, 3, p);
-                            const int n = sg.tile * 128 + row;
-                            const float nw = resid ? bf16_to_f32(nwp[n]) : 1.f;
-                            const float* base = a.scratch + (size_t)sg.slot0 * STEP_SCR_SLOT + row;
-                            // rank finishes batch rows rank, rank + KS, ...; the two warps of a lane group alternate over them
-                            for (int m = sg.rank + sg.ks * h; m < M; m += 2 * sg.ks) {
-                                float pv[2][STEP_KS_MAX];
-                                const float res = resid ? __ldcg(a.x + (size_t)m * a.d_model + n) : 0.f;
-#pragma unroll
-                                for (int na = 0; na < 2; ++na)
-#pragma unroll
-                                    for (int q = 0; q < STEP_KS_MAX; ++q)
-                                        pv[na][q] = (q < sg.ks && na < NA) ? __ldcg(base + (size_t)q * STEP_SCR_SLOT + ((size_t)na * 64 + m) * 128) : 0.f;
-                                float acc0 = pv[0][0], acc1 = pv[1][0];
-#pragma unroll
-                                for (int q = 1; q < STEP_KS_MAX; ++q) { acc0 += pv[0][q]; acc1 += pv[1][q]; }   // rank order: deterministic
-                                finish(ph, l, sg.tile, m, acc0, acc1, res, nw);
-                            }
-                            if (resid) {
-                                worker_sync();
-                                if (wt < M && (wt % sg.ks) == sg.rank)
-                                    a.ssq[(size_t)sg.tile * a.ssq_ld + wt] = sh->ssq_s[0][wt] + sh->ssq_s[1][wt] + sh->ssq_s[2][wt] + sh->ssq_s[3][wt];
-                                worker_sync();
-                            }
-                        }
-                    }
-                    tc_fence_before();
-                    step_trace(a, tron, 3, 4, p);
+                const int NA = a.g[ph].na;
+                const float* xin = (ph == 0) ? a.xa : a.xb;          // QKV reads xa (+ accD), gate/up reads xb (+ accO)
+                const long long* accin = (ph == 0) ? a.accD : a.accO;
+                const bf16_t* gain = (ph == 0) ? a.norm1[l] : a.norm2[l];
+                if (ph == 3) {
+                    if (wt < M) sh->rstd[wt] = __ldcg(a.rstd2 + wt);
+                    worker_sync();
                 }
+                // ---- build the B operand of every unit, one <= 32 KB chunk of k blocks at a time ----
+                for (int s = 0; s < nseg; ++s) {
+                    const StepSeg sg = sh->pl[ph].seg[s];
+                    for (int kc = sg.kb0; kc < sg.kb1; kc += CH, ++cn) {
+                        const int nk = min(CH, sg.kb1 - kc);
+                        const unsigned buf = cn & 1u, buse = cn >> 1;
+                        if (buse > 0) step_wait_mbar(&sh->bempty[buf], (buse - 1) & 1, a.err, 3);
+                        uint8_t* bb = att_kv + (size_t)buf * STEP_BBUF;
+                        const int tasks = M * nk * 8;                // (batch row, k block, 16-byte chunk)
+                        // two tasks per thread and iteration, every load of both issued before the first use
+                        for (int i0 = wt; i0 < tasks; i0 += 512) {
+                            int tc[2], tj[2], tm[2], tk[2];
+                            bool on[2];
+#pragma unroll
+                            for (int u = 0; u < 2; ++u) {
+                                const int i = i0 + 256 * u;
+                                on[u] = i < tasks;
+                                const int ii = on[u] ? i : i0;
+                                tc[u] = ii & 7; tj[u] = (ii >> 3) % nk; tm[u] = ii / (8 * nk);
+                                tk[u] = (kc + tj[u]) * 64 + tc[u] * 8;
+                            }
+                            if (ph == 1) {                            // attention output, already split: plain copy
+                                uint4 hi[2], lo[2];
+#pragma unroll
+                                for (int u = 0; u < 2; ++u) {
+                                    hi[u] = __ldcg(reinterpret_cast<const uint4*>(a.att_s + (size_t)(2 * tm[u]) * a.qd + tk[u]));
+                                    lo[u] = __ldcg(reinterpret_cast<const uint4*>(a.att_s + (size_t)(2 * tm[u] + 1) * a.qd + tk[u]));
+                                }
+#pragma unroll
+                                for (int u = 0; u < 2; ++u) {
+                                    if (!on[u]) continue;
+                                    uint8_t* tile = bb + (size_t)tj[u] * NB * 128;
+                                    const int r0 = 2 * tm[u], r1 = 2 * tm[u] + 1;
+                                    *reinterpret_cast<uint4*>(tile + (size_t)r0 * 128 + ((tc[u] ^ (r0 & 7)) << 4)) = hi[u];
+                                    *reinterpret_cast<uint4*>(tile + (size_t)r1 * 128 + ((tc[u] ^ (r1 & 7)) << 4)) = lo[u];
+                                }
+                            } else if (ph == 3) {                     // SwiGLU of the gate / up sums (1/rms applied here)
+                                float gt[2][8], up[2][8];
+#pragma unroll
+                                for (int u = 0; u < 2; ++u) {
+                                    load_fx8(a.accG + (size_t)tm[u] * 2 * F + tk[u], gt[u]);
+                                    load_fx8(a.accG + (size_t)tm[u] * 2 * F + F + tk[u], up[u]);
+                                }
+#pragma unroll
+                                for (int u = 0; u < 2; ++u) {
+                                    if (!on[u]) continue;
+                                    const float rs = sh->rstd[tm[u]];
+                                    float v[8];
+#pragma unroll
+                                    for (int e = 0; e < 8; ++e) v[e] = silu_f(gt[u][e] * rs) * (up[u][e] * rs);
+                                    store_b_chunk(bb + (size_t)tj[u] * NB * 128, tm[u], tc[u], v);
+                                }
+                            } else {                                  // (x + acc) * norm gain
+                                float xv[2][8], av[2][8], gv[2][8];
+#pragma unroll
+                                for (int u = 0; u < 2; ++u) {
+                                    load_f8(xin + (size_t)tm[u] * d + tk[u], xv[u]);
+                                    load_fx8(accin + (size_t)tm[u] * d + tk[u], av[u]);
+                                    load_bf8(gain + tk[u], gv[u]);
+                                }
+#pragma unroll
+                                for (int u = 0; u < 2; ++u) {
+                                    if (!on[u]) continue;
+                                    float v[8];
+#pragma unroll
+                                    for (int e = 0; e < 8; ++e) v[e] = (xv[u][e] + av[u][e]) * gv[u][e];
+                                    store_b_chunk(bb + (size_t)tj[u] * NB * 128, tm[u], tc[u], v);
+                                }
+                            }
+                        }
+                        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");   // generic-proxy smem writes -> tcgen05.mma reads
+                        worker_sync();
+                        if (wt == 0) mbar_arrive(&sh->bfull[buf]);
+                    }
+                }
+                step_trace(a, tron, 3, 1, p);
+                // ---- off the critical path: residual stream / 1/rms of the rows this CTA owns, accumulator recycling ----
+                if (ph == 0) { own_row(a.xa, a.accD, a.xb, a.rstd1); zero_acc(a.accG, 2 * F); }
+                if (ph == 1) zero_acc(a.accQ, a.Nqkv);
+                if (ph == 2) own_row(a.xb, a.accO, a.xa, a.rstd2);
+                if (ph == 3) zero_acc(a.accO, d);
+                // ---- drain: TMEM -> (hi + lo) -> fixed-point add into the phase's accumulator in L2 ----
+                long long* accout = (ph == 0) ? a.accQ : (ph == 1 ? a.accO : (ph == 2 ? a.accG : a.accD));
+                const int ldo = (ph == 0) ? a.Nqkv : (ph == 2 ? 2 * F : d);
+                for (int s = 0; s < nseg; ++s) {
+                    const StepSeg sg = sh->pl[ph].seg[s];
+                    step_wait_mbar(&sh->acc_full[s], acc_use[s] & 1, a.err, 7);
+                    ++acc_use[s];
+                    tc_fence_after();
+                    if (s == 0) step_trace(a, tron, 3, 2, p);
+                    for (int na = 0; na < NA; ++na) {
+                        const int n = sg.tile * 128 + row + na * F;          // gate rows, then up rows
+                        for (int c = h; c * 16 < M && c < NB / 32; c += 2) {
+                            float v[32];
+                            tc_ld32(tmem_base + ((uint32_t)(lg * 32) << 16) + (uint32_t)((s * 2 + na) * NB + c * 32), v);
+#pragma unroll
+                            for (int j = 0; j < 16; ++j) {
+                                const int m = c * 16 + j;
+                                if (m < M) red_add_fx(accout + (size_t)m * ldo + n, v[2 * j] + v[2 * j + 1]);
+                            }
+                        }
+                    }
+                }
+                tc_fence_before();
+                step_trace(a, tron, 3, 4, p);
                 arrive(p);
+            }
+        }
+        // ---- last phase: the LM-head operand of the rows this CTA owns (final residual, x * w_final split, sum of squares) ----
+        wait_phase(5 * L);
+        if (cta < M) {
+            const int m = cta;
+            float ss = 0.f;
+            for (int k = wt * 8; k < d; k += 2048) {
+                float xv[8], av[8], gv[8], v[8];
+                load_f8(a.xa + (size_t)m * d + k, xv);
+                load_fx8(a.accD + (size_t)m * d + k, av);
+                load_bf8(a.final_norm + k, gv);
+#pragma unroll
+                for (int e = 0; e < 8; ++e) { xv[e] += av[e]; ss += xv[e] * xv[e]; v[e] = xv[e] * gv[e]; }
+                *reinterpret_cast<float4*>(a.x + (size_t)m * d + k) = make_float4(xv[0], xv[1], xv[2], xv[3]);
+                *reinterpret_cast<float4*>(a.x + (size_t)m * d + k + 4) = make_float4(xv[4], xv[5], xv[6], xv[7]);
+                uint32_t hi[4], lo[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) split2(v[2 * i], v[2 * i + 1], hi[i], lo[i]);
+                *reinterpret_cast<uint4*>(a.xs + (size_t)(2 * m) * d + k) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+                *reinterpret_cast<uint4*>(a.xs + (size_t)(2 * m + 1) * d + k) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+            }
+            ss = warp_sum(ss);
+            if (lane == 0) sh->red[wi] = ss;
+            worker_sync();
+            if (wt == 0) {
+                float t = 0.f;
+                for (int i = 0; i < 8; ++i) t += sh->red[i];
+                a.ssq[m] = t;
+                for (int i = 1; i < a.d_tiles; ++i) a.ssq[(size_t)i * a.ssq_ld + m] = 0.f;
             }
         }
     }
     __syncthreads();
-    if (warp == 3) {
+    if (warp == 2) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "n"(512));
     }
@@ -584,16 +608,18 @@ int launch_decode_step(const StepLaunch& s, cudaStream_t st) {
     if (s.m_max <= 0 || s.m_max > 64 || (s.att.hd != 64 && s.att.hd != 128)) return -1;
     StepDev d = {};
     d.n_layers = s.n_layers; d.n_cta = s.n_cta; d.NB = 32 << tc_nb_index(s.m_max); d.n_slots = s.n_slots;
-    d.bper = STEP_SLOT / (d.NB * 128);
+    d.chunk = STEP_BBUF / (d.NB * 128);
     for (int i = 0; i < 4; ++i) d.g[i] = s.g[i];
     d.wmaps = reinterpret_cast<const CUtensorMap*>(s.wmaps_dev); d.plan = s.plan_dev;
-    d.x = s.x; d.qkv = s.qkv; d.xs = s.xs; d.att_s = s.att_s; d.act_s = s.act_s; d.ssq = s.ssq;
+    d.xa = s.xa; d.xb = s.xb; d.accQ = s.accQ; d.accO = s.accO; d.accG = s.accG; d.accD = s.accD; d.rstd1 = s.rstd1; d.rstd2 = s.rstd2;
+    d.x = s.x; d.xs = s.xs; d.att_s = s.att_s; d.ssq = s.ssq;
     d.ssq_ld = s.ssq_ld; d.d_tiles = s.d_tiles; d.d_model = s.d_model; d.Nqkv = s.Nqkv; d.qd = s.qd; d.d_ff = s.d_ff;
     d.norm1 = s.norm1_dev; d.norm2 = s.norm2_dev; d.final_norm = s.final_norm; d.embed = s.embed; d.eps = s.eps;
-    d.scratch = s.scratch; d.sync_base = s.sync_base; d.gbar_n = s.gbar_n; d.tcnt_n = s.tcnt_n; d.tiles_per_layer = s.tiles_per_layer;
+    d.sync_base = s.sync_base; d.gbar_n = s.gbar_n;
     d.live = s.live; d.pos = s.pos; d.ctx = s.ctx; d.tok = s.tok; d.n_live = s.n_live; d.step = s.step; d.m_max = s.m_max;
     d.att = s.att; d.kv_pool = s.kv_pool; d.layer_stride = s.layer_stride; d.err = s.err; d.trace = s.trace;
     { const char* e = getenv("SAGC_STEP_FLAGS"); d.flags = e ? atoi(e) : 0; }
+    { const char* e = getenv("SAGC_STEP_PREFETCH"); d.prefetch = e ? atoi(e) : 0; }
     const int smem = step_smem_bytes(s.n_slots);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(s.n_cta);
@@ -605,17 +631,13 @@ int launch_decode_step(const StepLaunch& s, cudaStream_t st) {
     if (s.cooperative) { at[na].id = cudaLaunchAttributeCooperative; at[na].val.cooperative = 1; ++na; }
     if (s.pdl) { at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[na].val.programmaticStreamSerializationAllowed = 1; ++na; }
     cfg.attrs = at; cfg.numAttrs = na;
-    const int nbi = tc_nb_index(s.m_max);
-    const CUtensorMap* bx = reinterpret_cast<const CUtensorMap*>(&s.bmaps[0][nbi]);
-    const CUtensorMap* ba = reinterpret_cast<const CUtensorMap*>(&s.bmaps[1][nbi]);
-    const CUtensorMap* bc = reinterpret_cast<const CUtensorMap*>(&s.bmaps[2][nbi]);
     cudaError_t e;
     if (s.att.hd == 128) {
         e = cudaFuncSetAttribute(k_decode_step<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e == cudaSuccess) e = cudaLaunchKernelEx(&cfg, k_decode_step<128>, *bx, *ba, *bc, d);
+        if (e == cudaSuccess) e = cudaLaunchKernelEx(&cfg, k_decode_step<128>, d);
     } else {
         e = cudaFuncSetAttribute(k_decode_step<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e == cudaSuccess) e = cudaLaunchKernelEx(&cfg, k_decode_step<64>, *bx, *ba, *bc, d);
+        if (e == cudaSuccess) e = cudaLaunchKernelEx(&cfg, k_decode_step<64>, d);
     }
     return e == cudaSuccess ? 1 : -1;
 }

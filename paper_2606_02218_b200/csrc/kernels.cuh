@@ -71,6 +71,9 @@ struct AttnArgs {
     // decode only (fuse_rope): q is the RAW qkv row; RoPE of q / k and the bf16 K,V append of the newest
     // position happen inside this kernel (no separate RoPE kernel).  head_dim >= 64.
     int fuse_rope; const float* rope_cs; const int* row_pos; bf16_t* kv_layer_w;
+    // decode-step kernel: the q | k | v row is a 64-bit fixed-point sum (value * 2^32, see decode_step.cu) that still
+    // lacks the 1/rms factor of its row; when q_fx is set it replaces q (same [row][ldq] indexing)
+    const long long* q_fx; const float* q_rstd;
     int prefetch;           // 1 in decode: cached positions older than the newest one predate the upstream kernel
     int cluster_merge;      // set by the launcher: the n_splits CTAs of a (row, kv head) form a cluster and merge through DSMEM
 };
@@ -91,6 +94,12 @@ struct SampleArgs {
 };
 int launch_sample(const SampleArgs& a, cudaStream_t st);
 int launch_philox_debug(uint64_t seed, int sid, int t, int v0, int n, uint32_t* out, cudaStream_t st);
+
+// Teacher-forced log-prob pass (row f4): row descriptors of prompt + generated tokens, and log-softmax at the target token.
+int launch_score_rows(const int* prompt_tokens, const int* prompt_offs_dev, const int* seq_off_dev, const int* gen_tokens, int nseq,
+                      int G, int max_new, int total, int* row_sid, int* row_pos, int* row_ctx, int* row_tok, cudaStream_t st);
+int launch_token_logprob(const float* logits, int V, int rows, const int* row_sid, const int* row_pos, const int* prompt_offs_dev, int G,
+                         const int* gen_tokens, int max_new, float* out, cudaStream_t st);
 
 // Segmented per-group statistics.  Step a14.
 int launch_group_advantage(const float* rewards, const int* offs, int n_groups, int mode, int ddof,
@@ -186,13 +195,14 @@ struct StepLaunch {
     StepGemm g[4];
     const void* wmaps_dev;                  // device CUtensorMap [n_layers][7]
     const StepPhasePlan* plan_dev;          // device [4][n_cta]
-    const TcMap (*bmaps)[4];                // host: {xs, att_s, act_s} x UMMA N {32, 64, 128, 256}
-    float* x; float* qkv; bf16_t* xs; bf16_t* att_s; bf16_t* act_s; float* ssq;
+    float* xa; float* xb;                   // fp32 residual stream ping-pong [64][d_model]
+    long long* accQ; long long* accO; long long* accG; long long* accD;   // fixed-point sums [64][Nqkv | d | 2 d_ff | d]
+    float* rstd1; float* rstd2;             // [64]
+    float* x; bf16_t* xs; bf16_t* att_s; float* ssq;
     int ssq_ld, d_tiles, d_model, Nqkv, qd, d_ff;
     const bf16_t* const* norm1_dev; const bf16_t* const* norm2_dev; const bf16_t* final_norm; const bf16_t* embed;
     float eps;
-    float* scratch;                         // >= 2 * n_cta * 2 * 64 * 128 floats
-    unsigned* sync_base; int gbar_n, tcnt_n, tiles_per_layer;
+    unsigned* sync_base; int gbar_n;        // [2][gbar_n] phase counters
     const int* live; const int* pos; const int* ctx; const int* tok; const int* n_live; const int* step;
     AttnArgs att;                           // everything but kv_layer / kv_layer_w (set per layer in the kernel)
     bf16_t* kv_pool; size_t layer_stride;

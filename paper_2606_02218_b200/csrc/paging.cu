@@ -259,7 +259,7 @@ __global__ void __launch_bounds__(PG_THREADS) k_advance(PageState ps, RolloutDev
         }
         *ps.n_free = n_free;
         *ps.n_retire += total_ret;
-        *ps.n_live = n_new;
+        *ps.n_live = exhausted ? 0 : n_new;      // pool exhausted: the remaining steps of the rollout see no live rows
         *ps.step = t + 1;
     }
 }

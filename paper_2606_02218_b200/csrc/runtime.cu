@@ -110,10 +110,12 @@ struct sagc_model {
     bool step_ok; int n_sm, step_slots, gbar_n, tcnt_n, tiles_per_layer;
     StepGemm step_g[4];
     void* wmaps_d; StepPhasePlan* plan_d; const bf16_t** norm1_d; const bf16_t** norm2_d; unsigned* step_sync; int* step_err;
-    bool step_coop;
+    float *step_xa, *step_xb, *step_rstd; long long *step_accQ, *step_accO, *step_accG, *step_accD;
+    bool step_coop; int step_max_rows;
     unsigned long long* step_trace;            // SAGC_STEP_TRACE=1: in-kernel timeline of one decode step (sagc_debug_step_trace)
     // host-buffer entry point: device staging buffers, grown on demand and kept by the handle
     int *h_prompt, *h_tok, *h_len, *h_stats; float* h_ratio; size_t h_prompt_cap, h_tok_cap, h_len_cap, h_grp_cap;
+    float* score_logits; size_t score_cap; int* seq_off_d; size_t seq_off_cap;    // teacher-forced log-prob pass
     cudaStream_t own_stream;                   // used when the caller passes the legacy default stream
     cudaEvent_t own_event;
 };
@@ -200,6 +202,7 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     m->row_sid = m->row_pos = m->row_ctx = m->row_tok = nullptr;
     m->h_prompt = m->h_tok = m->h_len = m->h_stats = nullptr; m->h_ratio = nullptr;
     m->h_prompt_cap = m->h_tok_cap = m->h_len_cap = m->h_grp_cap = 0;
+    m->score_logits = nullptr; m->score_cap = 0; m->seq_off_d = nullptr; m->seq_off_cap = 0;
     m->step_ok = false; m->n_sm = 0; m->step_trace = nullptr;
 
     DA(m->kv_pool, m->layer_stride * (size_t)(L > 0 ? L : 1));
@@ -289,14 +292,18 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
             cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
             m->step_slots = step_ring_slots(smem_optin);
             m->step_coop = env_int("SAGC_STEP_COOP", 1) != 0;
+            m->step_max_rows = env_int("SAGC_STEP_MAXROWS", 64);
             std::vector<StepPhasePlan> plan;
             if (m->tc_ok && env_int("SAGC_STEP", 1) != 0 && c.head_dim >= 64 && m->n_sm > 0 && m->step_slots >= 4 &&
                 build_step_plan(m->n_sm, c.d_model, qd, kvd, c.d_ff, m->step_g, plan, &m->tiles_per_layer)) {
-                m->gbar_n = 1 + 5 * L; m->tcnt_n = m->tiles_per_layer * L;
+                m->gbar_n = 2 + 5 * L; m->tcnt_n = 0;
                 unsigned char* wm = nullptr;
                 DA(wm, (size_t)L * 7 * sizeof(TcMap)); m->wmaps_d = wm;
                 DA(m->plan_d, plan.size()); DA(m->norm1_d, L); DA(m->norm2_d, L);
                 DA(m->step_sync, (size_t)2 * (m->gbar_n + m->tcnt_n)); DA(m->step_err, 1);
+                DA(m->step_xa, (size_t)64 * c.d_model); DA(m->step_xb, (size_t)64 * c.d_model); DA(m->step_rstd, 128);
+                DA(m->step_accQ, (size_t)64 * m->Nqkv); DA(m->step_accO, (size_t)64 * c.d_model);
+                DA(m->step_accG, (size_t)64 * 2 * c.d_ff); DA(m->step_accD, (size_t)64 * c.d_model);
                 cudaMemcpy(m->wmaps_d, m->wmaps.data(), (size_t)L * 7 * sizeof(TcMap), cudaMemcpyHostToDevice);
                 cudaMemcpy(m->plan_d, plan.data(), plan.size() * sizeof(StepPhasePlan), cudaMemcpyHostToDevice);
                 cudaMemcpy(m->norm1_d, m->norm1.data(), L * sizeof(void*), cudaMemcpyHostToDevice);
@@ -459,14 +466,16 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cuda
 #undef LAUNCH
 
 // final norm + LM head over rows of `xsrc` -> m->logits
-static int enqueue_lm_head(sagc_model* m, const float* xsrc, const int* m_dev, int m_max, int kind, cudaStream_t st) {
+static int enqueue_lm_head(sagc_model* m, const float* xsrc, const int* m_dev, int m_max, int kind, cudaStream_t st,
+                           float* Y = nullptr) {
     const sagc_model_config& c = m->cfg;
     if (m->skip_mask & 16) return 0;
+    if (!Y) Y = m->logits;
     if (kind == LIN_TC && xsrc == m->x) {
         // decode: the last down-projection left x * w_final pre-split in xs and its row sums in ssq
         TcLinearArgs t = {};
         t.a[0] = &m->wmaps[(size_t)c.n_layers * 7]; t.seg_rows[0] = c.vocab; t.b = &m->amaps[0][tc_nb_index(m_max)];
-        t.K = c.d_model; t.N = c.vocab; t.m_dev = m_dev; t.m_max = m_max; t.epi = EPI_STORE; t.Y = m->logits; t.ldy = c.vocab;
+        t.K = c.d_model; t.N = c.vocab; t.m_dev = m_dev; t.m_max = m_max; t.epi = EPI_STORE; t.Y = Y; t.ldy = c.vocab;
         t.ssq_in = m->ssq; t.ssq_in_tiles = m->d_tiles; t.ssq_ld = m->ssq_ld; t.eps = c.rms_eps; t.k_norm = c.d_model;
         t.pdl = m->use_pdl; t.scratch = m->tc_scratch;
         return launch_linear_tc(t, st);
@@ -474,7 +483,7 @@ static int enqueue_lm_head(sagc_model* m, const float* xsrc, const int* m_dev, i
     if (kind == LIN_TC) kind = LIN_MMA;          // gathered fp32 rows (first token): register HMMA path
     LinearArgs a = {};
     a.W[0] = m->lm_head; a.rows[0] = c.vocab; a.X = xsrc; a.norm_w = m->final_norm; a.eps = c.rms_eps;
-    a.Y = m->logits; a.ldy = c.vocab; a.K = c.d_model; a.N = c.vocab; a.m_dev = m_dev; a.m_max = m_max;
+    a.Y = Y; a.ldy = c.vocab; a.K = c.d_model; a.N = c.vocab; a.m_dev = m_dev; a.m_max = m_max;
     a.epi = EPI_STORE; a.kind = kind; a.pdl = m->use_pdl;
     return launch_linear(a, st);
 }
@@ -519,11 +528,14 @@ static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
 // ---------------------------------------------------------------------------------------
 // the persistent decode-step kernel covers the tcgen05 path at <= 64 live rows (head_dim 64 / 128)
 static bool step_kernel_applies(const sagc_model* m, int kind, int m_bucket) {
-    return m->step_ok && kind == LIN_TC && m_bucket <= 64 && m->skip_mask == 0;
+    return m->step_ok && kind == LIN_TC && m_bucket <= m->step_max_rows && m->skip_mask == 0;
 }
 
 static int enqueue_decode_step(sagc_model* m, const RolloutDev& rd, int m_bucket, int n_splits, int kind,
-                               int n_dump, float* dump_out, cudaStream_t st) {
+                               int n_dump, float* dump_out, cudaStream_t st, std::vector<cudaEvent_t>* evs = nullptr) {
+    // SAGC_FLAG_TIME_KERNELS: four events per step bracket the layer stack, the LM head + sampler and the advance kernel
+    auto stamp = [&]() { if (evs) { cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, st); evs->push_back(e); } };
+    stamp();
     RowSet rs = {m->ps.live, m->ps.pos, m->ps.ctx, m->ps.tok, m->ps.n_live, m_bucket};
     const sagc_model_config& c = m->cfg;
     int n;
@@ -532,14 +544,17 @@ static int enqueue_decode_step(sagc_model* m, const RolloutDev& rd, int m_bucket
         StepLaunch s = {};
         s.n_layers = c.n_layers; s.n_cta = m->n_sm; s.n_slots = m->step_slots; s.m_max = m_bucket;
         for (int i = 0; i < 4; ++i) s.g[i] = m->step_g[i];
-        s.wmaps_dev = m->wmaps_d; s.plan_dev = m->plan_d; s.bmaps = m->amaps;
-        s.x = m->x; s.qkv = m->qkv; s.xs = m->xs; s.att_s = m->att_s; s.act_s = m->act_s; s.ssq = m->ssq;
+        s.wmaps_dev = m->wmaps_d; s.plan_dev = m->plan_d;
+        s.xa = m->step_xa; s.xb = m->step_xb; s.accQ = m->step_accQ; s.accO = m->step_accO; s.accG = m->step_accG; s.accD = m->step_accD;
+        s.rstd1 = m->step_rstd; s.rstd2 = m->step_rstd + 64;
+        s.x = m->x; s.xs = m->xs; s.att_s = m->att_s; s.ssq = m->ssq;
         s.ssq_ld = m->ssq_ld; s.d_tiles = m->d_tiles; s.d_model = c.d_model; s.Nqkv = m->Nqkv; s.qd = c.n_q_heads * c.head_dim; s.d_ff = c.d_ff;
         s.norm1_dev = m->norm1_d; s.norm2_dev = m->norm2_d; s.final_norm = m->final_norm; s.embed = m->embed; s.eps = c.rms_eps;
-        s.scratch = m->tc_scratch; s.sync_base = m->step_sync; s.gbar_n = m->gbar_n; s.tcnt_n = m->tcnt_n; s.tiles_per_layer = m->tiles_per_layer;
+        s.sync_base = m->step_sync; s.gbar_n = m->gbar_n;
         s.live = m->ps.live; s.pos = m->ps.pos; s.ctx = m->ps.ctx; s.tok = m->ps.tok; s.n_live = m->ps.n_live; s.step = m->ps.step;
         AttnArgs& aa = s.att;
-        aa.q = m->qkv; aa.ldq = m->Nqkv; aa.page_table = m->ps.page_table; aa.max_blocks = m->max_blocks; aa.row_sid = m->ps.live;
+        aa.q = nullptr; aa.q_fx = m->step_accQ; aa.q_rstd = m->step_rstd; aa.ldq = m->Nqkv; aa.page_table = m->ps.page_table;
+        aa.max_blocks = m->max_blocks; aa.row_sid = m->ps.live;
         aa.row_ctx = m->ps.ctx; aa.m_dev = m->ps.n_live; aa.m_max = m_bucket; aa.Hq = c.n_q_heads; aa.Hkv = c.n_kv_heads; aa.hd = c.head_dim;
         aa.page = c.page_tokens; aa.n_splits = 1; aa.part_o = m->part_o; aa.part_ml = m->part_ml; aa.counters = m->counters; aa.out = m->att;
         aa.out_split = m->att_s; aa.ld_split = c.n_q_heads * c.head_dim; aa.fuse_rope = 1; aa.rope_cs = m->rope_cs; aa.row_pos = m->ps.pos;
@@ -551,6 +566,7 @@ static int enqueue_decode_step(sagc_model* m, const RolloutDev& rd, int m_bucket
         n = enqueue_layers(m, rs, n_splits, kind, st);
     }
     if (n < 0) return -1;
+    stamp();
     if (m->lm_fused && kind == LIN_TC && m_bucket <= 64 && n_dump == 0 && (c.vocab % 128) == 0 && !(m->skip_mask & (2 | 16))) {
         // a11 + a12 in one persistent kernel: the logits never reach HBM
         LmSampleArgs f = {};
@@ -561,7 +577,9 @@ static int enqueue_decode_step(sagc_model* m, const RolloutDev& rd, int m_bucket
         int r = launch_lmhead_sample(f, st);
         if (r < 0) return -1;
         n += r;
+        stamp();
         n += launch_advance(m->ps, rd, m->lm_score, m->lm_tok, 0, st, lm_sample_grid(c.vocab), 64, 1);
+        stamp();
         return n;
     }
     int r = enqueue_lm_head(m, m->x, m->ps.n_live, m_bucket, kind, st);
@@ -575,7 +593,9 @@ static int enqueue_decode_step(sagc_model* m, const RolloutDev& rd, int m_bucket
     if (n_dump > 0)
         n += launch_dump_logits(m->dump_list_d, n_dump, m->ps.step, m->ps.live, m->ps.n_live, 1, m->logits,
                                 m->cfg.vocab, dump_out, st);
+    stamp();
     n += launch_advance(m->ps, rd, m->part_score, m->sampled, 0, st);
+    stamp();
     return n;
 }
 
@@ -606,7 +626,9 @@ extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, c
     const int nseq = n_prompts * G;
     const int max_new = prm->max_new_tokens;
     const bool structure_only = (prm->flags & SAGC_FLAG_STRUCTURE_ONLY) != 0;
-    const bool use_graph = !(prm->flags & SAGC_FLAG_NO_GRAPH);
+    const bool time_kernels = (prm->flags & SAGC_FLAG_TIME_KERNELS) != 0 && timing != nullptr;
+    const bool use_graph = !(prm->flags & SAGC_FLAG_NO_GRAPH) && !time_kernels;
+    std::vector<cudaEvent_t> kev;
     if (n_prompts < 1 || G < 1 || nseq > c.max_seqs) return set_err(SAGC_EINVAL, "n_prompts*G = %d exceeds max_seqs = %d", nseq, c.max_seqs);
     if (max_new < 1) return set_err(SAGC_EINVAL, "max_new_tokens must be >= 1");
     if (structure_only && !prm->forced_lengths) return set_err(SAGC_EINVAL, "STRUCTURE_ONLY needs forced_lengths");
@@ -681,16 +703,24 @@ extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, c
     int t_last = 0;
     for (int i = 0; i < nseq; ++i) if (eff[i] > t_last) t_last = eff[i];
     std::vector<int> live_at(t_last + 2, 0), glive_at;     // live_at[t] = #{eff >= t}
+    std::vector<double> gplen_at;                          // sum of the prompt lengths of the groups still live at step t
     {
         std::vector<int> cnt(t_last + 2, 0);
         for (int i = 0; i < nseq; ++i) cnt[eff[i]]++;
         int run = 0;
         for (int t = t_last; t >= 1; --t) { run += cnt[t]; live_at[t] = run; }
         glive_at.assign(t_last + 2, 0);
+        gplen_at.assign(t_last + 2, 0.0);
         std::vector<int> gcnt(t_last + 2, 0);
-        for (int p = 0; p < n_prompts; ++p) { int mx = 0; for (int g = 0; g < G; ++g) mx = eff[p * G + g] > mx ? eff[p * G + g] : mx; gcnt[mx]++; }
+        std::vector<double> gpl(t_last + 2, 0.0);
+        for (int p = 0; p < n_prompts; ++p) {
+            int mx = 0;
+            for (int g = 0; g < G; ++g) mx = eff[p * G + g] > mx ? eff[p * G + g] : mx;
+            gcnt[mx]++; gpl[mx] += plen[p];
+        }
         run = 0;
-        for (int t = t_last; t >= 1; --t) { run += gcnt[t]; glive_at[t] = run; }
+        double prun = 0.0;
+        for (int t = t_last; t >= 1; --t) { run += gcnt[t]; glive_at[t] = run; prun += gpl[t]; gplen_at[t] = prun; }
     }
     const bool known = prm->forced_lengths != nullptr && prm->stop_token < 0;
 
@@ -709,6 +739,14 @@ extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, c
     if (want_t) e_start = mark();
 
     if (!structure_only) {
+        // a pool too small for the prefixes leaves the page tables unmapped: stop before any kernel walks them
+        int perr = 0;
+        CU(cudaMemcpyAsync(&perr, m->ps.err, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        if (perr) {
+            for (int i = 0; i < n_ev; ++i) cudaEventDestroy(ev[i]);
+            return set_err(SAGC_EPAGES, "KV page pool exhausted by the prompt prefixes (n_pages = %d)", c.n_pages);
+        }
         // ---- a2: prefill, once per prompt, in row chunks ----------------------------------
         const int* ptok = prompt_tokens;      // device pointer supplied by the caller
         launches += launch_prefill_rows(ptok, m->offs_d, n_prompts, G, total_rows, m->row_sid, m->row_pos, m->row_ctx,
@@ -767,6 +805,12 @@ extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, c
         if (known) {
             if (t > t_last) break;
             live = live_at[t];
+            if (!structure_only && (t & 255) == 0) {      // a pool exhausted mid-rollout ends it early (k_advance publishes 0 live rows)
+                int herr2 = 0;
+                CU(cudaMemcpyAsync(&herr2, m->ps.err, sizeof(int), cudaMemcpyDeviceToHost, st));
+                CU(cudaStreamSynchronize(st));
+                if (herr2) break;
+            }
         } else {
             if (t > max_new) break;
             if ((t - 2) % 16 == 0) {          // poll the device's live count
@@ -790,8 +834,8 @@ extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, c
         if (want_t) {
             timing->phase_steps[ph] += 1;
             timing->phase_tokens[ph] += live;
-            const double gl = known ? glive_at[t] : n_prompts;
-            timing->phase_bytes[ph] += Wb + KVB * (gl * (double)pmax + (double)live * (t - 1)) + KVB * live;
+            const double prefix = known ? gplen_at[t] : (double)total_rows;      // stop-token mode: every group counted until the end
+            timing->phase_bytes[ph] += Wb + KVB * (prefix + (double)live * (t - 1)) + KVB * live;
         }
         if (structure_only) {
             launches += launch_advance(m->ps, rd, m->part_score, m->sampled, 1, st);
@@ -821,7 +865,7 @@ extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, c
                 CU(cudaGraphLaunch(it->second.exec, st));
                 launches += it->second.n_kernels;
             } else {
-                r = enqueue_decode_step(m, rd, mb, ns, kind, prm->n_dump, prm->dump_logits, st);
+                r = enqueue_decode_step(m, rd, mb, ns, kind, prm->n_dump, prm->dump_logits, st, time_kernels ? &kev : nullptr);
                 if (r < 0) return set_err(SAGC_ECUDA, "decode launch failed: %s", cudaGetErrorString(cudaGetLastError()));
                 launches += r;
             }
@@ -856,11 +900,22 @@ extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, c
         timing->prefill_tokens = structure_only ? 0 : total_rows;
         timing->prefill_flops = structure_only ? 0.0 : (double)total_rows * Wb;   // 2 flop per bf16 weight per row (+attention, not counted)
         long long tot = 0;
-        for (int i = 0; i < nseq; ++i) tot += known ? eff[i] : 0;
+        if (known) {
+            for (int i = 0; i < nseq; ++i) tot += eff[i];
+        } else {                                  // stop-token mode: the lengths are only known on the device
+            std::vector<int> hl(nseq);
+            CU(cudaMemcpy(hl.data(), m->len_buf, (size_t)nseq * sizeof(int), cudaMemcpyDeviceToHost));
+            for (int i = 0; i < nseq; ++i) tot += hl[i];
+        }
         timing->total_tokens = tot;
         timing->kernel_launches = launches;
+        for (size_t i = 0; i + 3 < kev.size(); i += 4) {
+            for (int k = 0; k < 3; ++k) { cudaEventElapsedTime(&ms, kev[i + k], kev[i + k + 1]); timing->kernel_ms[k] += ms; }
+            timing->kernel_steps += 1;
+        }
     }
     for (int i = 0; i < n_ev; ++i) cudaEventDestroy(ev[i]);
+    for (cudaEvent_t e : kev) cudaEventDestroy(e);
     if (herr) return set_err(SAGC_EPAGES, "KV page pool exhausted (n_pages = %d)", c.n_pages);
     return SAGC_OK;
 }
@@ -875,30 +930,97 @@ extern "C" int sagc_rollout_group_host(sagc_model* m, const int32_t* prompt_toke
     if (n_prompts < 1 || G < 1 || prm->max_new_tokens < 1) return set_err(SAGC_EINVAL, "bad sizes");
     const size_t ntok = (size_t)nseq * prm->max_new_tokens;
     const int total = prompt_offsets[n_prompts];
-    int *d_prompt = nullptr, *d_tok = nullptr, *d_len = nullptr, *d_stats = nullptr;
-    float* d_ratio = nullptr;
-    int rc = SAGC_OK;
-    auto fail = [&](int code) {
-        cudaFree(d_prompt); cudaFree(d_tok); cudaFree(d_len); cudaFree(d_stats); cudaFree(d_ratio);
-        return code;
-    };
-#define CUH(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return fail(set_err(SAGC_ECUDA, "%s: %s", #x, cudaGetErrorString(e_))); } while (0)
-    CUH(cudaMalloc(&d_prompt, (size_t)(total > 0 ? total : 1) * sizeof(int)));
-    CUH(cudaMalloc(&d_tok, ntok * sizeof(int)));
-    CUH(cudaMalloc(&d_len, (size_t)nseq * sizeof(int)));
-    CUH(cudaMalloc(&d_stats, (size_t)n_prompts * 3 * sizeof(int)));
-    CUH(cudaMalloc(&d_ratio, (size_t)n_prompts * sizeof(float)));
+    int rc;
+    // device staging buffers live in the handle (grown on demand): no cudaMalloc / cudaFree in the timed call
+    if ((rc = grow(m, &m->h_prompt, &m->h_prompt_cap, (size_t)(total > 0 ? total : 1), nullptr)) != SAGC_OK) return rc;
+    if ((rc = grow(m, &m->h_tok, &m->h_tok_cap, ntok, nullptr)) != SAGC_OK) return rc;
+    if ((rc = grow(m, &m->h_len, &m->h_len_cap, (size_t)nseq, nullptr)) != SAGC_OK) return rc;
+    if ((size_t)n_prompts > m->h_grp_cap || !m->h_stats) {
+        size_t c1 = 0, c2 = 0;
+        m->h_stats = nullptr; m->h_ratio = nullptr;
+        if ((rc = grow(m, &m->h_stats, &c1, (size_t)n_prompts * 3, nullptr)) != SAGC_OK) return rc;
+        if ((rc = grow(m, &m->h_ratio, &c2, (size_t)n_prompts, nullptr)) != SAGC_OK) return rc;
+        m->h_grp_cap = (size_t)n_prompts;
+    }
     if (prompt_tokens && total > 0)
-        CUH(cudaMemcpyAsync(d_prompt, prompt_tokens, (size_t)total * sizeof(int), cudaMemcpyHostToDevice, st));
-    rc = sagc_rollout_group(m, prompt_tokens ? d_prompt : nullptr, prompt_offsets, n_prompts, G, prm, d_tok, d_len,
-                            d_ratio, d_stats, timing, stream);
-    if (rc != SAGC_OK) return fail(rc);
-    CUH(cudaMemcpyAsync(out_tokens, d_tok, ntok * sizeof(int), cudaMemcpyDeviceToHost, st));
-    CUH(cudaMemcpyAsync(out_lengths, d_len, (size_t)nseq * sizeof(int), cudaMemcpyDeviceToHost, st));
-    if (out_ratio) CUH(cudaMemcpyAsync(out_ratio, d_ratio, (size_t)n_prompts * sizeof(float), cudaMemcpyDeviceToHost, st));
-    if (out_len_stats) CUH(cudaMemcpyAsync(out_len_stats, d_stats, (size_t)n_prompts * 3 * sizeof(int), cudaMemcpyDeviceToHost, st));
-    CUH(cudaStreamSynchronize(st));
-    fail(0);
+        CU(cudaMemcpyAsync(m->h_prompt, prompt_tokens, (size_t)total * sizeof(int), cudaMemcpyHostToDevice, st));
+    rc = sagc_rollout_group(m, prompt_tokens ? m->h_prompt : nullptr, prompt_offsets, n_prompts, G, prm, m->h_tok, m->h_len,
+                            m->h_ratio, m->h_stats, timing, stream);
+    if (rc != SAGC_OK) return rc;
+    CU(cudaMemcpyAsync(out_tokens, m->h_tok, ntok * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(out_lengths, m->h_len, (size_t)nseq * sizeof(int), cudaMemcpyDeviceToHost, st));
+    if (out_ratio) CU(cudaMemcpyAsync(out_ratio, m->h_ratio, (size_t)n_prompts * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (out_len_stats) CU(cudaMemcpyAsync(out_len_stats, m->h_stats, (size_t)n_prompts * 3 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return SAGC_OK;
+}
+
+
+// ---------------------------------------------------------------------------------------
+// sagc_score_tokens: teacher-forced log-prob pass
+// ---------------------------------------------------------------------------------------
+extern "C" int sagc_score_tokens(sagc_model* m, const int32_t* prompt_tokens, const int32_t* prompt_offsets, int32_t n_prompts, int32_t G,
+                                 const int32_t* tokens, const int32_t* lengths, int32_t max_new, float* out_logprobs, void* stream) {
+    if (!m || !prompt_tokens || !prompt_offsets || !tokens || !lengths || !out_logprobs) return set_err(SAGC_EINVAL, "null argument");
+    const sagc_model_config& c = m->cfg;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const int nseq = n_prompts * G;
+    if (n_prompts < 1 || G < 1 || nseq > c.max_seqs || max_new < 1) return set_err(SAGC_EINVAL, "bad sizes (n_prompts*G <= max_seqs)");
+    if (c.n_layers < 1) return set_err(SAGC_EINVAL, "model has no layers");
+    std::vector<int> seq_off(nseq + 1, 0), seq_len(nseq);
+    long long pages = 0;
+    for (int sid = 0; sid < nseq; ++sid) {
+        const int P = prompt_offsets[sid / G + 1] - prompt_offsets[sid / G];
+        const int ell = lengths[sid];
+        if (P < 1 || ell < 1 || ell > max_new || P + ell > c.max_ctx) return set_err(SAGC_EINVAL, "sequence %d: bad prompt / completion length", sid);
+        seq_len[sid] = P + ell - 1;                    // the last generated token is only a target
+        seq_off[sid + 1] = seq_off[sid] + seq_len[sid];
+        pages += (seq_len[sid] + c.page_tokens - 1) / c.page_tokens;
+    }
+    if (pages > c.n_pages) return set_err(SAGC_EPAGES, "scoring needs %lld KV pages, the pool has %d", pages, c.n_pages);
+    const int total_rows = seq_off[nseq];
+    int rc;
+    bool changed = false;
+    if ((rc = grow(m, &m->tok_buf, &m->tok_cap, (size_t)nseq * max_new, &changed)) != SAGC_OK) return rc;
+    if (!m->len_buf) { size_t cap = 0; if ((rc = grow(m, &m->len_buf, &cap, (size_t)c.max_seqs, &changed)) != SAGC_OK) return rc; }
+    if ((size_t)total_rows > (size_t)m->row_cap) {
+        size_t c1 = 0, c2 = 0, c3 = 0, c4 = 0;
+        m->row_sid = m->row_pos = m->row_ctx = m->row_tok = nullptr;
+        if ((rc = grow(m, &m->row_sid, &c1, (size_t)total_rows, &changed)) != SAGC_OK) return rc;
+        if ((rc = grow(m, &m->row_pos, &c2, (size_t)total_rows, &changed)) != SAGC_OK) return rc;
+        if ((rc = grow(m, &m->row_ctx, &c3, (size_t)total_rows, &changed)) != SAGC_OK) return rc;
+        if ((rc = grow(m, &m->row_tok, &c4, (size_t)total_rows, &changed)) != SAGC_OK) return rc;
+        m->row_cap = (int)c1;
+    }
+    if ((rc = grow(m, &m->score_logits, &m->score_cap, (size_t)PREFILL_ROWS * c.vocab, &changed)) != SAGC_OK) return rc;
+    if ((rc = grow(m, &m->seq_off_d, &m->seq_off_cap, (size_t)nseq + 1, &changed)) != SAGC_OK) return rc;
+    if (changed) { clear_graphs(m); m->signature.clear(); }          // the rollout graphs bake tok_buf / row buffers
+    CU(cudaMemcpyAsync(m->seq_off_d, seq_off.data(), (nseq + 1) * sizeof(int), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(m->prompt_len_d, seq_len.data(), nseq * sizeof(int), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(m->offs_d, prompt_offsets, (n_prompts + 1) * sizeof(int), cudaMemcpyHostToDevice, st));
+    CU(cudaMemsetAsync(out_logprobs, 0, (size_t)nseq * max_new * sizeof(float), st));
+    // every sequence is its own "prompt" of length P + l - 1 (G = 1): the paging kernels lay its KV out in fresh pages
+    RolloutDev rd = {};
+    rd.prompt_len = m->prompt_len_d; rd.out_tokens = m->tok_buf; rd.out_lengths = m->len_buf;
+    rd.n_prompts = nseq; rd.G = 1; rd.nseq = nseq; rd.max_new = max_new; rd.stop_token = -1;
+    launch_pool_reset(m->ps, rd, st);
+    launch_prefill_alloc(m->ps, rd, st);
+    launch_score_rows(prompt_tokens, m->offs_d, m->seq_off_d, tokens, nseq, G, max_new, total_rows, m->row_sid, m->row_pos, m->row_ctx,
+                      m->row_tok, st);
+    const int kind = pick_kind(m, SAGC_PATH_AUTO, PREFILL_ROWS);
+    for (int r0 = 0; r0 < total_rows; r0 += PREFILL_ROWS) {
+        const int rows = (total_rows - r0) < PREFILL_ROWS ? (total_rows - r0) : PREFILL_ROWS;
+        RowSet rs = {m->row_sid + r0, m->row_pos + r0, m->row_ctx + r0, m->row_tok + r0, nullptr, rows};
+        if (enqueue_layers(m, rs, 1, kind, st) < 0) return set_err(SAGC_ECUDA, "scoring: layer launch failed");
+        if (enqueue_lm_head(m, m->x, nullptr, rows, kind, st, m->score_logits) < 0) return set_err(SAGC_ECUDA, "scoring: LM head launch failed");
+        launch_token_logprob(m->score_logits, c.vocab, rows, m->row_sid + r0, m->row_pos + r0, m->offs_d, G, tokens, max_new, out_logprobs, st);
+    }
+    int herr = 0;
+    CU(cudaMemcpyAsync(&herr, m->ps.err, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    m->last_nseq = nseq;
+    if (herr) return set_err(SAGC_EPAGES, "KV page pool exhausted (n_pages = %d)", c.n_pages);
     return SAGC_OK;
 }
 

@@ -118,4 +118,69 @@ int launch_dump_logits(const int* dump_sid_t, int n_dump, const int* step_dev, c
     return 1;
 }
 
+// ---- teacher-forced log-prob pass (row f4) ------------------------------------------------------------------
+// Row descriptors: sequence sid = prompt tokens of its group followed by its own generated tokens but the last;
+// rows of all sequences are concatenated (seq_off).  row r of sid at offset j: pos = j, ctx = j + 1.
+__global__ void k_score_rows(const int* __restrict__ prompt_tokens, const int* __restrict__ prompt_offs, const int* __restrict__ seq_off,
+                             const int* __restrict__ gen_tokens, int nseq, int G, int max_new, int total, int* row_sid, int* row_pos,
+                             int* row_ctx, int* row_tok) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= total) return;
+    int lo = 0, hi = nseq;               // largest sid with seq_off[sid] <= r
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (seq_off[mid] <= r) lo = mid; else hi = mid;
+    }
+    const int sid = lo, j = r - seq_off[sid], p = sid / G;
+    const int P = prompt_offs[p + 1] - prompt_offs[p];
+    row_sid[r] = sid; row_pos[r] = j; row_ctx[r] = j + 1;
+    row_tok[r] = j < P ? prompt_tokens[prompt_offs[p] + j] : gen_tokens[(size_t)sid * max_new + (j - P)];
+}
+int launch_score_rows(const int* prompt_tokens, const int* prompt_offs_dev, const int* seq_off_dev, const int* gen_tokens, int nseq,
+                      int G, int max_new, int total, int* row_sid, int* row_pos, int* row_ctx, int* row_tok, cudaStream_t st) {
+    if (total <= 0) return 0;
+    k_score_rows<<<(total + 255) / 256, 256, 0, st>>>(prompt_tokens, prompt_offs_dev, seq_off_dev, gen_tokens, nseq, G, max_new, total,
+                                                      row_sid, row_pos, row_ctx, row_tok);
+    return 1;
+}
+
+// log pi(y_t | x, y_<t) = logit[y_t] - logsumexp(logits) for every row that predicts a generated token:
+// row (sid, pos) with pos >= P - 1 predicts token t = pos - (P - 1) (0-based).  One CTA per row; fp32, max-subtracted.
+__global__ void __launch_bounds__(256) k_token_logprob(const float* __restrict__ logits, int V, const int* __restrict__ row_sid,
+                                                        const int* __restrict__ row_pos, const int* __restrict__ prompt_offs, int G,
+                                                        const int* __restrict__ gen_tokens, int max_new, float* __restrict__ out) {
+    __shared__ float red[8];
+    const int r = blockIdx.x;
+    const int sid = row_sid[r], pos = row_pos[r], p = sid / G;
+    const int P = prompt_offs[p + 1] - prompt_offs[p];
+    if (pos < P - 1) return;
+    const int t = pos - (P - 1);
+    const float* lg = logits + (size_t)r * V;
+    float mx = -INFINITY;
+    for (int v = threadIdx.x; v < V; v += 256) mx = fmaxf(mx, lg[v]);
+    mx = warp_max(mx);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mx;
+    __syncthreads();
+    mx = red[0];
+    for (int i = 1; i < 8; ++i) mx = fmaxf(mx, red[i]);
+    __syncthreads();
+    float sum = 0.f;
+    for (int v = threadIdx.x; v < V; v += 256) sum += __expf(lg[v] - mx);
+    sum = warp_sum(sum);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = sum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float tot = 0.f;
+        for (int i = 0; i < 8; ++i) tot += red[i];
+        const int tok = gen_tokens[(size_t)sid * max_new + t];
+        out[(size_t)sid * max_new + t] = lg[tok] - mx - logf(tot);
+    }
+}
+int launch_token_logprob(const float* logits, int V, int rows, const int* row_sid, const int* row_pos, const int* prompt_offs_dev, int G,
+                         const int* gen_tokens, int max_new, float* out, cudaStream_t st) {
+    if (rows <= 0) return 0;
+    k_token_logprob<<<rows, 256, 0, st>>>(logits, V, row_sid, row_pos, prompt_offs_dev, G, gen_tokens, max_new, out);
+    return 1;
+}
+
 }  // namespace sagc

@@ -201,3 +201,47 @@ def test_rollout_256_live_rows_through_every_bucket(B, mode):
                 n_dis += 1
                 n_bad += oph.top2_margin(s) >= 1e-2
     assert n_bad == 0 and n_dis <= 0.005 * n_all, (n_bad, n_dis, n_all)
+
+
+@pytest.mark.parametrize("shape", ["tiny_gqa", "cfg2"])
+def test_score_tokens_vs_oracle(B, shape):
+    """f4: sagc_score_tokens = log pi(y_t | x, y_<t) of every generated token in ONE
+    causal pass per sequence (prefill kernels + LM head over every position) vs the oracle's float64 log-softmax of its
+    teacher-forced logits.  Tolerance: 2 x the 3e-2 logit bar (a log-prob is a logit minus a log-sum-exp of logits)."""
+    if shape == "tiny_gqa":
+        w = wl.tiny_variant(1, model_n_q_heads=8, model_n_kv_heads=2, model_head_dim=64, model_d_model=256, model_d_ff=768,
+                            model_n_layers=3, model_vocab=2048, model_page_tokens=16)
+        weights = wl.make_weights(w.model, 1)
+        plens, G, max_new = [7, 16, 41, 2300], 3, 40          # the last prompt spans two 2 048-row chunks
+        lens = np.array([1, 40, 17, 16, 9, 33, 25, 2, 40, 5, 12, 30], dtype=np.int32)
+        check = range(len(plens) * G)
+    else:
+        w = wl.WORKLOADS[2]
+        weights = wl.make_weights(w.model, 0)
+        plens, G, max_new = [256, 100], 2, 24
+        lens = np.array([24, 3, 11, 24], dtype=np.int32)
+        check = [0, 3]
+    offs = np.concatenate([[0], np.cumsum(plens)]).astype(np.int32)
+    rng = np.random.default_rng(33)
+    prompts = rng.integers(0, w.model.vocab, size=offs[-1]).astype(np.int32)
+    nseq = len(plens) * G
+    toks = -np.ones((nseq, max_new), dtype=np.int32)
+    for sid in range(nseq):
+        toks[sid, :lens[sid]] = rng.integers(0, w.model.vocab, size=lens[sid])
+    page = w.model.page_tokens
+    n_pages = sum((plens[sid // G] + int(lens[sid]) + page - 1) // page for sid in range(nseq)) + 4
+    m = B.Model(w.model, weights, n_pages, nseq, max(plens) + max_new)
+    lp = m.score_tokens(prompts, offs, G, torch.from_numpy(toks).cuda(), lens).cpu().numpy()
+    # the handle is still good for a rollout afterwards (the pass reuses its KV pool and page tables)
+    out = m.rollout_group(prompts[:offs[1]], offs[:2], 2, mode=B.MODE_GREEDY, max_new_tokens=4)
+    assert out.lengths.cpu().numpy().tolist() == [4, 4]
+    m.close()
+    dec = odec.RefDecoder(w.model, weights)
+    worst = 0.0
+    for sid in check:
+        p = sid // G
+        L = int(lens[sid])
+        ref = oro.token_logprobs(dec, prompts[offs[p]:offs[p + 1]], toks[sid, :L])
+        worst = max(worst, float(np.max(np.abs(lp[sid, :L] - ref))))
+        assert np.all(lp[sid, L:] == 0.0)
+    assert worst <= 6e-2, worst

@@ -374,3 +374,34 @@ def test_fused_lm_head_sampler_gives_identical_tokens(B, monkeypatch, G, mode, c
     for a, b in zip(outs[0], outs[1]):
         assert np.array_equal(a, b)
     assert (outs[0][0] >= 0).sum() == int(fl.sum())
+
+
+def test_sagc_controller_closes_the_loop_on_the_gpu(B):
+    """f1 + f3 (Alg.1 l.173-210, sec 5.2 l.216-218): the CPU-side controller picks G, every rollout step is one
+    sagc_rollout_group call with B_t = 16 / G_t prompts on one handle, and the (max, sum, median_x2) triples that come
+    back from the GPU -- the only thing the controller needs (l.153-157) -- equal the oracle's on the same lengths."""
+    from paper_2606_02218_b200.controller import SAGCController, run_sagc
+    w = wl.tiny_variant(1)
+    weights = wl.make_weights(w.model, 0)
+    prompts_all, _ = wl.make_prompts(w, n_prompts=4, prompt_len=24)
+    m = B.Model(w.model, weights, 600, 16, 24 + 32)
+    rng = np.random.default_rng(12)
+    seen = []
+
+    def step(t, G, n_prompts):
+        offs = (np.arange(n_prompts + 1) * 24).astype(np.int32)
+        fl = np.clip(np.rint(12 * np.exp(0.25 * rng.standard_normal(n_prompts * G))), 1, 32).astype(np.int32)
+        out = m.rollout_group(prompts_all[: n_prompts * 24], offs, G, mode=B.MODE_GUMBEL, seed=900 + t, max_new_tokens=32,
+                              forced_lengths=fl)
+        st = out.len_stats.cpu().numpy()
+        st_o, _ = ogs.length_stats(fl, np.arange(n_prompts + 1) * G)
+        assert np.array_equal(st, st_o)
+        seen.append((G, n_prompts))
+        return st
+
+    c = SAGCController([2, 4, 8, 16], delta=0.4, eta_lambda=0.5, gamma=0.9, seed=2, g0=4)
+    log = run_sagc(step, c, 12, effective_batch=16)
+    m.close()
+    assert all(g * b == 16 for g, b in seen)
+    assert all(abs(c.sizes.index(r["next_G"]) - c.sizes.index(r["G"])) <= 1 for r in log)
+    assert all(r["lambda"] >= 0 for r in log)

@@ -169,3 +169,30 @@ def test_rollout_gumbel_teacher_forced_consistency():
     for row, t in zip(lg, (1, 5, 10)):
         assert np.allclose(row, res.logits[(0, t)], atol=2e-5)
         assert philox.sample_token(row, 1, 1.0, 4001, 0, t) == res.tokens[0, t - 1]
+
+
+def test_token_logprobs_pins():
+    """oracle.rollout.token_logprobs: (i) library routine: scipy.special.log_softmax of the same logits; (ii) invariant:
+    the log-probs over the whole vocabulary of one position sum to 1 in probability; (iii) brute force: a sequence's
+    log-likelihood equals the sum of the step-by-step cached-decode log-softmax values."""
+    oro = rollout
+    w = wl.WORKLOADS[1]
+    weights = wl.make_weights(w.model, 0)
+    dec = od.RefDecoder(w.model, weights)
+    rng = np.random.default_rng(0)
+    prompt = rng.integers(0, w.model.vocab, size=9)
+    gen = rng.integers(0, w.model.vocab, size=7)
+    lp = oro.token_logprobs(dec, prompt, gen)
+    assert lp.shape == (7,) and np.all(lp < 0)
+    scipy_special = pytest.importorskip("scipy.special")
+    lg = oro.teacher_forced_logits(dec, prompt, gen, list(range(1, 8))).astype(np.float64)
+    ref = scipy_special.log_softmax(lg, axis=1)
+    assert np.allclose(lp, ref[np.arange(7), gen], atol=1e-12)
+    assert np.allclose(np.exp(ref).sum(axis=1), 1.0, atol=1e-12)
+    # brute force through the cached decode path
+    lg0, cache = dec.prefill(prompt)
+    rows = [lg0]
+    for t in range(1, 7):
+        rows.append(dec.step(int(gen[t - 1]), len(prompt) + t - 1, cache))
+    step_lp = [float(scipy_special.log_softmax(r.astype(np.float64))[gen[t]]) for t, r in enumerate(rows)]
+    assert np.allclose(lp, step_lp, atol=2e-4)
