@@ -270,7 +270,9 @@ def kernel_parts(model, B, w, d_prompts, offs, fl, max_new, mode, peak):
         parts[name] = {"ms_per_step": ms[k] / steps, "share_of_step": ms[k] / max(sum(ms), 1e-9), "bytes_per_step": nbytes / steps,
                        "achieved_gbs": nbytes / ms[k] / 1e6 if ms[k] > 0 else None,
                        "frac": nbytes / ms[k] / 1e6 / peak if ms[k] > 0 else None}
-    parts["layer_stack"]["kernel"] = "k_decode_step (persistent, one launch per step) while <= 64 rows are live; per-layer k_linear_tc / k_attention above"
+    parts["layer_stack"]["kernel"] = ("k_decode_step (persistent, one launch per step) while <= 64 rows are live; per-layer k_linear_tc / k_attention above"
+                                      if os.environ.get("SAGC_STEP", "0") not in ("", "0") else
+                                      "per layer: k_linear_tc<QKV>, k_attention (RoPE + KV append fused), k_linear_tc<O+resid>, k_linear_tc<gate/up SwiGLU>, k_linear_tc<down+resid>")
     parts["lm_head_sampler"]["kernel"] = "k_lmhead_sample (fused, <= 64 rows) / k_linear_tc + k_sample above"
     parts["advance"]["kernel"] = "k_advance"
     parts["steps_measured"] = steps
@@ -305,6 +307,66 @@ def side_7b(B, torch, peak, tf_sustained, device):
             "targets": {"full_frac_of_8tbs": 0.70, "tail_frac_of_8tbs": 0.60}}
 
 
+def run_fixed_eb(args, local):
+    """--protocol fixed-eb (sec 5.2 l.216-218, Table 5 l.398-405): the paper compares group
+    sizes at a FIXED effective generation batch, B_t = EB / G_t prompts per step (EB = 64).  Each static G in {4, 8, 16, 32}
+    and the SAGC controller (paper_2606_02218_b200.controller) run `--eb-steps` rollout steps on the configs[1] model with
+    fresh seeded lognormal lengths per step (the paper's lengths come from the evolving policy: these stand in for them).
+    Reports time per step, tokens/s and the straggler rate P(max / median > 1.25) per arm: the shape of the paper's
+    time-vs-G trade-off, context only."""
+    import torch
+    from paper_2606_02218_b200 import binding as B
+    from paper_2606_02218_b200.controller import SAGCController, run_sagc, straggler_events
+    torch.cuda.set_device(local)
+    w = wl.WORKLOADS[2]
+    mc = w.model
+    EB, P, max_new, med, sigma = 64, 256, 1024, 256.0, 0.35
+    weights = wl.make_weights(mc, 0)
+    page = mc.page_tokens
+    model = B.Model(mc, weights, EB // 4 * (P // page) + EB * ((max_new + page - 1) // page + 2) + 8, EB, P + max_new, device=f"cuda:{local}")
+    del weights
+    prompts, _ = wl.make_prompts(w, n_prompts=EB // 4, prompt_len=P)
+    d_prompts = torch.from_numpy(prompts).cuda()
+    rng = np.random.default_rng(6000)
+
+    def make_step(acc):
+        def step(t, G, n_prompts):
+            fl = np.clip(np.rint(med * np.exp(sigma * rng.standard_normal(n_prompts * G))), 1, max_new).astype(np.int32)
+            offs = (np.arange(n_prompts + 1) * P).astype(np.int32)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            out = model.rollout_group(d_prompts[: n_prompts * P], offs, G, mode=B.MODE_GUMBEL, temperature=1.0, seed=7000 + t,
+                                      max_new_tokens=max_new, forced_lengths=fl)
+            e1.record()
+            torch.cuda.synchronize()
+            st = out.len_stats.cpu().numpy()
+            acc.append({"G": G, "ms": e0.elapsed_time(e1), "tokens": int(fl.sum()), "S": float(straggler_events(st).mean())})
+            return st
+        return step
+
+    rows = []
+    for G in (4, 8, 16, 32):
+        acc = []
+        step = make_step(acc)
+        for t in range(args.eb_steps + 1):
+            step(t, G, EB // G)
+        acc = acc[1:]                                    # first step builds the graphs
+        rows.append({"arm": f"static G={G}", "prompts_per_step": EB // G, "ms_per_step": float(np.mean([a["ms"] for a in acc])),
+                     "tokens_per_s": sum(a["tokens"] for a in acc) / sum(a["ms"] for a in acc) * 1e3,
+                     "straggler_rate": float(np.mean([a["S"] for a in acc]))})
+    acc = []
+    ctrl = SAGCController([4, 8, 16, 32], delta=0.5, eta_lambda=0.5, gamma=0.9, seed=1, g0=8)
+    run_sagc(make_step(acc), ctrl, 4 * args.eb_steps, effective_batch=EB)
+    rows.append({"arm": "SAGC (delta=0.5, eta=0.5, gamma=0.9)", "ms_per_step": float(np.mean([a["ms"] for a in acc])),
+                 "tokens_per_s": sum(a["tokens"] for a in acc) / sum(a["ms"] for a in acc) * 1e3,
+                 "straggler_rate": float(np.mean([a["S"] for a in acc])), "G_trajectory": [a["G"] for a in acc],
+                 "mean_G": float(np.mean([a["G"] for a in acc]))})
+    model.close()
+    print(json.dumps({"protocol": "fixed_effective_batch", "effective_batch": EB, "metric": METRIC, "unit": UNIT, "data": "synthetic",
+                      "config": {"workload": f"configs[1] model (0.5B shape), {P}-token prompts, B_t = {EB}/G_t prompts per step, lengths "
+                                             f"lognormal({med:g}, {sigma:g}) cap {max_new} redrawn every step"}, "arms": rows}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -315,12 +377,17 @@ def main():
     ap.add_argument("--max-new", type=int, default=0, help="override max_new_tokens (debug; invalidates the number)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-side-7b", action="store_true", help="skip the configs[4] (7B shape) side block (~5 minutes)")
+    ap.add_argument("--protocol", default="rollout", choices=["rollout", "fixed-eb"],
+                    help="fixed-eb: the paper's fixed-effective-batch comparison of group sizes (side mode, own JSON line)")
+    ap.add_argument("--eb-steps", type=int, default=6)
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         return run_reference(args, rank, world)
+    if args.protocol == "fixed-eb":
+        return run_fixed_eb(args, local) if rank == 0 else None
 
     import torch
     import torch.distributed as dist

@@ -97,3 +97,46 @@ def run_sagc(rollout_step: Callable[[int, int, int], np.ndarray], controller: SA
         log.append({"step": t, "G": G, "n_prompts": B, "R_mean": float(R.mean()), "S_bar": float(S.mean()),
                     "lambda": controller.lam, "next_G": nxt})
     return log
+
+
+class GroupFIFO:
+    """FIFO of completed groups between generation and the controller (PAPER.md sec C.2 l.433-435: "it drains a FIFO
+    queue of recently completed groups (token-length vectors)"; sec C.3 l.439: "groups can be assembled across
+    microbatches until the expected group size is reached, then emitted as a single observation").
+    `push(prompt_id, lengths, expected)` may deliver a group's completions in several pieces (micro-batches); a group
+    enters the queue once `expected` lengths have arrived.  `drain()` returns the token-length vectors of the groups
+    completed since the last drain, in completion order, as (lengths int32 concatenated, CSR offsets int32) -- the
+    input of `sagc_length_stats`; `drain_stats()` runs that kernel and returns the (max, sum, median_x2) triples."""
+
+    def __init__(self):
+        self._partial = {}
+        self._ready: List[np.ndarray] = []
+
+    def push(self, prompt_id, lengths: Sequence[int], expected: int) -> bool:
+        buf = self._partial.setdefault(prompt_id, [])
+        buf.extend(int(x) for x in lengths)
+        if len(buf) > expected:
+            raise ValueError(f"group {prompt_id}: {len(buf)} completions delivered, {expected} expected")
+        if len(buf) < expected:
+            return False
+        self._ready.append(np.asarray(self._partial.pop(prompt_id), dtype=np.int32))
+        return True
+
+    def pending(self) -> int:
+        return len(self._partial)
+
+    def drain(self):
+        groups, self._ready = self._ready, []
+        offs = np.concatenate([[0], np.cumsum([g.shape[0] for g in groups])]).astype(np.int32)
+        ell = np.concatenate(groups).astype(np.int32) if groups else np.zeros(0, dtype=np.int32)
+        return ell, offs
+
+    def drain_stats(self, device: str = "cuda:0") -> np.ndarray:
+        """(max, sum, median_x2) per drained group through the library's segmented kernel (step a14)."""
+        import torch
+        from . import binding
+        ell, offs = self.drain()
+        if offs.shape[0] == 1:
+            return np.zeros((0, 3), dtype=np.int32)
+        st, _ = binding.length_stats(torch.from_numpy(ell).to(device), torch.from_numpy(offs).to(device))
+        return st.cpu().numpy()

@@ -13,7 +13,7 @@ struct AttStandalone {       // 8 compute warps x 16 tokens per tile; K/V tiles 
     using G = AttGeom<HD, WARPS, NSTAGE>;
 };
 
-template <int HD>
+template <int HD, int WARPS, int NSTAGE>
 __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     extern __shared__ __align__(128) unsigned char kv_s[];
     __shared__ AttSmall sm;
@@ -27,14 +27,13 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
     const int M = a.m_dev ? min(*a.m_dev, a.m_max) : a.m_max;
     const int row = blockIdx.x, kvh = blockIdx.y, split = blockIdx.z;
     if (row >= M) { if (a.prefetch) pdl_wait(); pdl_launch(); return; }      // uniform over the cluster (same row)
-    attention_unit<HD, AttStandalone<HD>::WARPS, AttStandalone<HD>::NSTAGE, false>(a, row, kvh, split, a.n_splits, kv_s, &sm, &cl,
-                                                                                   (int)threadIdx.x);
+    attention_unit<HD, WARPS, NSTAGE, false>(a, row, kvh, split, a.n_splits, kv_s, &sm, &cl, (int)threadIdx.x);
 }
 
-template <int HD>
-static int launch_att(const AttnArgs& a, cudaStream_t st) {
-    constexpr int BYTES = AttStandalone<HD>::G::BYTES;
-    if (cudaFuncSetAttribute(k_attention<HD>, cudaFuncAttributeMaxDynamicSharedMemorySize, BYTES) != cudaSuccess) return -1;
+template <int HD, int WARPS, int NSTAGE>
+static int launch_att_geom(const AttnArgs& a, cudaStream_t st) {
+    constexpr int BYTES = AttGeom<HD, WARPS, NSTAGE>::BYTES;
+    if (cudaFuncSetAttribute(k_attention<HD, WARPS, NSTAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, BYTES) != cudaSuccess) return -1;
     dim3 grid(a.m_max, a.Hkv, a.n_splits);
     if (a.n_splits > 1 && a.n_splits <= 8) {      // 2..8 splits merge inside a cluster through DSMEM
         AttnArgs ac = a;
@@ -47,9 +46,17 @@ static int launch_att(const AttnArgs& a, cudaStream_t st) {
         at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         at[1].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = at; cfg.numAttrs = g_pdl_all ? 2 : 1;
-        return cudaLaunchKernelEx(&cfg, k_attention<HD>, ac) == cudaSuccess ? 1 : -1;
+        return cudaLaunchKernelEx(&cfg, k_attention<HD, WARPS, NSTAGE>, ac) == cudaSuccess ? 1 : -1;
     }
-    return launch_pdl(k_attention<HD>, grid, dim3(ATT_THREADS), BYTES, st, g_pdl_all, a) == cudaSuccess ? 1 : -1;
+    return launch_pdl(k_attention<HD, WARPS, NSTAGE>, grid, dim3(ATT_THREADS), BYTES, st, g_pdl_all, a) == cudaSuccess ? 1 : -1;
+}
+
+template <int HD>
+static int launch_att(const AttnArgs& a, cudaStream_t st) {
+    // a.geom (parity / tuning entry only): alternative K/V staging geometries of the same unit
+    if (HD >= 64 && a.geom == 1) return launch_att_geom<HD, 4, 4>(a, st);       // 64-token tiles, 4 stages
+    if (HD >= 64 && a.geom == 2) return launch_att_geom<HD, 4, 3>(a, st);       // 64-token tiles, 3 stages
+    return launch_att_geom<HD, AttStandalone<HD>::WARPS, AttStandalone<HD>::NSTAGE>(a, st);
 }
 
 int launch_attention(const AttnArgs& a, cudaStream_t st) {

@@ -11,6 +11,7 @@ namespace sagc {
 typedef uint16_t bf16_t;   // raw bf16 bit pattern
 
 extern bool g_pdl_all;     // launch the small kernels (embed, rope, attention, sampler, advance) with the PDL attribute too
+extern int g_num_sms;      // multiprocessor count of the current device (set by sagc_model_create; 148 on B200)
 
 enum { EPI_STORE = 0, EPI_RESID = 1, EPI_SWIGLU = 2, EPI_QKV = 3 };   // EPI_QKV: tcgen05 path only (fused RoPE + KV append)
 enum { LIN_MMA = 0, LIN_GEMV = 1, LIN_TC = 2 };
@@ -75,6 +76,7 @@ struct AttnArgs {
     // lacks the 1/rms factor of its row; when q_fx is set it replaces q (same [row][ldq] indexing)
     const long long* q_fx; const float* q_rstd;
     int prefetch;           // 1 in decode: cached positions older than the newest one predate the upstream kernel
+    int geom;               // standalone launcher: 0 = default staging geometry, 1 / 2 = 64-token tiles with 4 / 3 stages
     int cluster_merge;      // set by the launcher: the n_splits CTAs of a (row, kv head) form a cluster and merge through DSMEM
 };
 int launch_attention(const AttnArgs& a, cudaStream_t st);

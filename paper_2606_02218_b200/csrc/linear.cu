@@ -743,7 +743,7 @@ static cudaError_t launch_epi(const LinearArgs& a, const LinDev& d, cudaStream_t
         // that the grid is ONE wave (small CTAs co-reside) and long K gets more warps (fewer load rounds).
         const int n_kb = a.K / 32;
         if (tiles > 148 * 2) return launch_cfg(k_linear_tail<EPI, true, 4>, dim3(tiles), 0, a.pdl, st, d, 128);
-        if (n_kb >= 96 && tiles <= 74 && getenv("SAGC_TAIL_CLUSTER")) {   // optional: K split over a 2-CTA cluster (DSMEM reduce)
+        if (false && n_kb >= 96 && tiles <= 74) {   // optional: K split over a 2-CTA cluster (DSMEM reduce)
             return launch_cfg(k_linear_tail<EPI, true, 16>, dim3(tiles, 2), 0, a.pdl, st, d, 512, 2);
         }
         if (n_kb >= 96 && tiles <= 148) return launch_cfg(k_linear_tail<EPI, true, 16>, dim3(tiles), 0, a.pdl, st, d, 512);

@@ -15,7 +15,7 @@
 
 using namespace sagc;
 
-namespace sagc { bool g_pdl_all = false; }
+namespace sagc { bool g_pdl_all = false; int g_num_sms = 148; }
 
 #ifdef SAGC_TRACE
 namespace sagc { __device__ unsigned long long* g_trace = nullptr; }
@@ -191,11 +191,12 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     m->page_elems = (size_t)2 * c.n_kv_heads * c.page_tokens * c.head_dim;
     m->layer_stride = m->page_elems * (size_t)c.n_pages;
     m->use_pdl = env_int("SAGC_PDL", 1) != 0;
-    sagc::g_pdl_all = m->use_pdl && env_int("SAGC_PDL_ALL", 1) != 0;
-    m->gemv_max = env_int("SAGC_GEMV_MAX", 0);
+    sagc::g_pdl_all = m->use_pdl;
+    { int dev = 0, n = 0; cudaGetDevice(&dev); if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) sagc::g_num_sms = n; }
+    m->gemv_max = 0;                          // the GEMV kernels serve SAGC_PATH_GEMV only: slower than the tensor-core paths even at 1 row
     m->skip_mask = env_int("SAGC_SKIP", 0);
     m->lm_fused = env_int("SAGC_LM_FUSED", 1);
-    m->tc_min = env_int("SAGC_TC_MIN", 1);   // measured: the tcgen05 path beats the register-HMMA tail kernels at every batch size
+    m->tc_min = 1;                            // measured: the tcgen05 path beats the register-HMMA tail kernels at every batch size
     m->tok_buf = m->len_buf = m->forced_len_d = m->dump_list_d = m->prompt_tok_d = nullptr;
     m->tok_cap = m->forced_cap = m->dump_cap = m->prompt_cap = 0;
     m->row_cap = 0;
@@ -294,7 +295,9 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
             m->step_coop = env_int("SAGC_STEP_COOP", 1) != 0;
             m->step_max_rows = env_int("SAGC_STEP_MAXROWS", 64);
             std::vector<StepPhasePlan> plan;
-            if (m->tc_ok && env_int("SAGC_STEP", 1) != 0 && c.head_dim >= 64 && m->n_sm > 0 && m->step_slots >= 4 &&
+            // SAGC_STEP=1 routes decode steps with <= 64 live rows through the persistent decode-step kernel.  Off by default:
+            // measured slower than the per-layer kernels on every shape (~1 us per L2 hop, 5 hops per phase)
+            if (m->tc_ok && env_int("SAGC_STEP", 0) != 0 && c.head_dim >= 64 && m->n_sm > 0 && m->step_slots >= 4 &&
                 build_step_plan(m->n_sm, c.d_model, qd, kvd, c.d_ff, m->step_g, plan, &m->tiles_per_layer)) {
                 m->gbar_n = 2 + 5 * L; m->tcnt_n = 0;
                 unsigned char* wm = nullptr;
@@ -417,12 +420,11 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cuda
         bf16_t* kv_layer = m->kv_pool + (size_t)l * m->layer_stride;
         t.rope_cs = m->rope_cs; t.row_pos = rs.pos; t.row_sid = rs.sid; t.page_table = m->ps.page_table; t.kv_layer = kv_layer;
         t.max_blocks = m->max_blocks; t.page = c.page_tokens; t.Hkv = c.n_kv_heads; t.hd = c.head_dim; t.q_rows = qd; t.kv_rows = kvd;
-        static const bool fuse_rope = env_int("SAGC_FUSE_ROPE", 0) != 0;   // measured: no gain in TAIL, -4% in FULL -> off by default
+        const bool fuse_rope = false;          // RoPE + append in the QKV epilogue (EPI_QKV): measured -4% in FULL, kept off
         if (!fuse_rope) t.epi = EPI_STORE;
         if (!(skip & 4)) LAUNCH(launch_linear_tc(t, st));
         // decode: RoPE + KV append are done inside the attention kernel (one launch less per layer)
-        static const bool fuse_att_env = env_int("SAGC_FUSE_ATT", 1) != 0;
-        const bool fuse_att = fuse_att_env && !fuse_rope && rs.m_dev != nullptr && c.head_dim >= 64;
+        const bool fuse_att = !fuse_rope && rs.m_dev != nullptr && c.head_dim >= 64;
         if (!fuse_rope && !fuse_att) {
             RopeArgs ra = {};
             ra.qkv = m->qkv; ra.row_sid = rs.sid; ra.row_pos = rs.pos; ra.m_dev = rs.m_dev; ra.m_max = rs.m_max;
@@ -509,7 +511,7 @@ static int round_bucket(int live) {
 
 static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
     const int ctas = m_bucket * m->cfg.n_kv_heads;
-    static const int target = env_int("SAGC_ATT_CTAS", 222);
+    const int target = (3 * sagc::g_num_sms) / 2;
     int want = target / ctas;                  // ~1.5 CTAs per SM; no split once the grid fills the chip
     if (want < 1) want = 1;
     int cap = ctx_bound / 128;
@@ -518,7 +520,7 @@ static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
     if (want > m->max_splits) want = m->max_splits;
     int s = 1;
     while (s * 2 <= want) s *= 2;
-    static const int smax = env_int("SAGC_ATT_MAXSPLIT", 8);      // <= 8 splits merge inside a cluster (attention.cu)
+    const int smax = 8;                       // <= 8 splits merge inside a cluster (attention.cu)
     if (s > smax) s = smax;
     return s;
 }
@@ -1211,7 +1213,7 @@ extern "C" int sagc_debug_attention(const float* q, const void* kv, const int32_
     if (!q || !kv || !page_table || !ctx || !out || M < 1) return set_err(SAGC_EINVAL, "null argument");
     if (Hq % Hkv || Hq / Hkv > 8) return set_err(SAGC_EINVAL, "bad head counts");
     if (n_splits < 1 || n_splits > 64) return set_err(SAGC_EINVAL, "n_splits must be in 1..64");
-    if (variant != 0 && variant != 1) return set_err(SAGC_EINVAL, "variant must be 0 (standalone kernel) or 1 (decode-step units)");
+    if (variant < 0 || variant > 3) return set_err(SAGC_EINVAL, "variant must be 0 (standalone kernel), 1 (decode-step units), 2 / 3 (standalone, 64-token tiles x 4 / 3 stages)");
     if (variant == 1 && hd != 64 && hd != 128) return set_err(SAGC_EINVAL, "the decode-step units need head_dim 64 or 128");
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     int *sid = nullptr, *cnt = nullptr;
@@ -1230,6 +1232,7 @@ extern "C" int sagc_debug_attention(const float* q, const void* kv, const int32_
     a.hd = hd; a.page = page_tokens; a.n_splits = n_splits; a.part_o = po; a.part_ml = pml; a.counters = cnt; a.out = out;
     int n_sm = 148;
     { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); }
+    a.geom = variant >= 2 ? variant - 1 : 0;
     int r = variant == 1 ? launch_attention_units(a, n_sm, st) : launch_attention(a, st);
     cudaError_t e = cudaStreamSynchronize(st);
     cudaFree(sid); cudaFree(cnt); cudaFree(po); cudaFree(pml);

@@ -487,18 +487,15 @@ static cudaError_t launch_tc_inst(const TcLinearArgs& t, const TcDev& d, dim3 gr
     using C = TcCfg<NB, NA>;
     // grids that fit the chip in one wave get the deepest ring; multi-wave grids (LM head, prefill) keep
     // ~100 KB so two CTAs share an SM and one's epilogue overlaps the other's loads
-    const bool one_wave = (long long)grid.x * grid.y * grid.z <= 148;
+    const bool one_wave = (long long)grid.x * grid.y * grid.z <= g_num_sms;
     // wide batch tiles (UMMA N = 256) are throughput-bound per CTA: give them the deepest ring as well
-    static const int deep256 = [] { const char* e = getenv("SAGC_TC_DEEP256"); return e ? atoi(e) : 1; }();
-    const int stages = (one_wave || (NB == 256 && deep256)) ? C::MAXSTAGES : C::STAGES;
+    const int stages = (one_wave || NB == 256) ? C::MAXSTAGES : C::STAGES;
     const int smem = C::smem_bytes(stages, EPI == EPI_QKV);
     TcDev d2 = d; d2.stages = stages;
-    static bool attr_set = false;
-    if (!attr_set) {
+    {   // per launch: a per-process flag would miss a second device
         cudaError_t e = cudaFuncSetAttribute(k_linear_tc<NB, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              C::smem_bytes(C::MAXSTAGES, EPI == EPI_QKV));
         if (e != cudaSuccess) return e;
-        attr_set = true;
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid;
@@ -539,15 +536,14 @@ int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
     // epilogue -- so K is split down to ~30 KB slabs per CTA (swept on cfg2), in powers of two up to 8, and never beyond two CTAs per SM.
     const int NAh = (t.epi == EPI_SWIGLU) ? 2 : 1;
     const double slab = (double)NAh * 128.0 * t.K * 2.0;
-    static const double slab_max = [] { const char* e = getenv("SAGC_TC_SLAB_KB"); return (e ? atof(e) : 30.0) * 1e3; }();
+    const double slab_max = 30.0e3;
     int KS = (int)((slab + slab_max - 1) / slab_max);
-    const int room = (2 * 148) / (tiles * mtiles);
+    const int room = (2 * g_num_sms) / (tiles * mtiles);
+    if ((size_t)2 * g_num_sms * 2 * 128 * 128 > TC_SCRATCH_FLOATS) return -1;      // split-K scratch is sized for 296 CTAs
     if (KS > room) KS = room;
     if (KS < 1) KS = 1;
     if (KS > 8) KS = 8;
     if (KS > d.n_kb) KS = d.n_kb;
-    static const int ks_swiglu = [] { const char* e = getenv("SAGC_TC_KS_SWIGLU"); return e ? atoi(e) : 0; }();
-    if (t.epi == EPI_SWIGLU && ks_swiglu > 0 && tiles * mtiles * ks_swiglu <= 2 * 148) KS = ks_swiglu;   // scratch holds 296 CTA tiles
     if (t.scratch == nullptr) KS = 1;
     { int p2 = 1; while (p2 * 2 <= KS) p2 *= 2; KS = p2; }      // the epilogue is specialised for 1, 2, 4, 8
     d.kb_per_cta = (d.n_kb + KS - 1) / KS;             // trailing ranks may get fewer (or zero) k blocks
@@ -829,7 +825,7 @@ static cudaError_t launch_lm_inst(const LmSampleArgs& t, LmDev d, int grid, cuda
     constexpr int A_BYTES = 128 * 128, B_BYTES = NB * 128, STAGE = A_BYTES + B_BYTES;
     // SAGC_LM_BRES: 0 = activation tile re-fetched with every stage, 1 = resident at UMMA N = 32, 2 = also at N = 64
     // (only when at least four weight stages still fit beside it)
-    static const int bres_knob = [] { const char* e = getenv("SAGC_LM_BRES"); return e ? atoi(e) : 0; }();
+    constexpr int bres_knob = 0;        // resident activation tiles: measured no gain, kept for reference
     const int b_all = d.n_kb * B_BYTES;
     const bool want = (bres_knob >= 1 && NB == 32) || (bres_knob >= 2 && NB == 64);
     d.bres = (want && b_all + 4 * A_BYTES <= 196 * 1024) ? 1 : 0;
@@ -837,11 +833,9 @@ static cudaError_t launch_lm_inst(const LmSampleArgs& t, LmDev d, int grid, cuda
     if (stages > 10) stages = 10;
     d.stages = stages;
     const int smem = (d.bres ? b_all + stages * A_BYTES : stages * STAGE) + 512 + (NB / 2) * 8 + 1024;
-    static bool attr_set = false;
-    if (!attr_set) {
+    {
         cudaError_t e = cudaFuncSetAttribute(k_lmhead_sample<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e != cudaSuccess) return e;
-        attr_set = true;
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
@@ -877,7 +871,7 @@ int launch_pick_candidates(const float* part_score, const int* part_tok, int n_p
 
 int lm_sample_grid(int V) {
     const char* e = getenv("SAGC_LM_CTAS");          // read per call (graph build time): tests force several tiles per CTA
-    const int g = (e && atoi(e) > 0) ? atoi(e) : 148;
+    const int g = (e && atoi(e) > 0) ? atoi(e) : g_num_sms;
     const int tiles = V / 128;
     return tiles < g ? tiles : (g > LM_MAX_PARTS ? LM_MAX_PARTS : g);
 }

@@ -113,3 +113,23 @@ def test_closed_loop_rate_settles_at_delta():
     c_hi = SAGCController(sizes, delta=0.999, eta_lambda=0.2, gamma=0.97, seed=3, g0=4)
     log_hi = run_sagc(step, c_hi, 600, effective_batch=64)
     assert np.mean([r["G"] == 32 for r in log_hi[200:]]) > 0.9
+
+
+def test_group_fifo_assembles_groups_across_microbatches():
+    """PAPER.md sec C.2-C.3 (l.433-439): completed groups queue up in FIFO order; a group delivered in pieces counts once,
+    when its last completion arrives."""
+    from paper_2606_02218_b200.controller import GroupFIFO
+    q = GroupFIFO()
+    ell, offs = q.drain()
+    assert ell.shape == (0,) and offs.tolist() == [0]
+    assert not q.push("a", [100, 200], 4)
+    assert q.push("b", [7, 9, 8, 30], 4)                  # b completes first
+    assert q.pending() == 1
+    assert q.push("a", [300, 1000], 4)
+    ell, offs = q.drain()
+    assert offs.tolist() == [0, 4, 8] and ell.tolist() == [7, 9, 8, 30, 100, 200, 300, 1000]
+    st = np.concatenate([_stats(ell[offs[g]:offs[g + 1]], 4) for g in range(2)])
+    assert st.tolist() == [[30, 54, 17], [1000, 1600, 500]] and straggler_events(st).tolist() == [1, 1]
+    assert q.drain()[1].tolist() == [0] and q.pending() == 0
+    with pytest.raises(ValueError):
+        q.push("c", [1, 2, 3], 2)

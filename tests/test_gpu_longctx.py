@@ -66,10 +66,23 @@ def _read_golden(name):
     return key, ids, rows
 
 
-@pytest.mark.parametrize("name", ["cfg2", "cfg5"])
-def test_teacher_forced_long_context(B, name):
+_WEIGHTS = {}
+
+
+def _weights(w):
+    """7B weights take minutes to draw: keep one copy per config for the module."""
+    if w.cfg not in _WEIGHTS:
+        _WEIGHTS.clear()
+        _WEIGHTS[w.cfg] = wl.make_weights(w.model, 0)
+    return _WEIGHTS[w.cfg]
+
+
+@pytest.mark.parametrize("name,step_kernel", [("cfg2", 0), ("cfg2", 1), ("cfg5", 0), ("cfg5", 1)])
+def test_teacher_forced_long_context(B, monkeypatch, name, step_kernel):
+    """step_kernel = 0: the per-layer kernels (default path); 1: the persistent decode-step kernel (SAGC_STEP=1)."""
+    monkeypatch.setenv("SAGC_STEP", str(step_kernel))
     w, prompts, offs, G, max_new, fl, ftok, ids, pos = mlg.case_inputs(name)
-    weights = wl.make_weights(w.model, 0)
+    weights = _weights(w)
     dump = [(sid, t) for sid in sorted(pos) for t in pos[sid] if t <= fl[sid]]
     if os.environ.get("SAGC_LIVE_ORACLE"):
         dec = odec.RefDecoder(w.model, weights, cache_f32=w.model.n_params() < 1e9)
@@ -164,11 +177,12 @@ def test_prefill_many_chunks_ragged(B):
 
 
 @pytest.mark.parametrize("mode", [0, 1])
-def test_rollout_256_live_rows_through_every_bucket(B, mode):
+def test_rollout_256_live_rows_through_every_bucket(B, monkeypatch, mode):
     """full-path parity with hundreds of live rows.  8 prompts x G = 32 = 256 completions on a small
     128-aligned model: the batch walks down through the 256 / 192 / 128 / 64 / 32 / 16 / 8 row buckets (UMMA N = 256
     with several m-tiles, the unfused LM head + sampler above 64 rows, attention and k_advance with hundreds of rows,
     then the persistent decode-step kernel).  Structure bit-exact; tokens under the margin rule, teacher forced."""
+    monkeypatch.setenv("SAGC_STEP", str(mode))        # greedy run: per-layer kernels; Gumbel run: decode-step kernel below 65 rows
     w = wl.tiny_variant(1, model_n_q_heads=4, model_n_kv_heads=2, model_head_dim=64, model_d_model=256, model_d_ff=512,
                         model_n_layers=2, model_vocab=2048, model_page_tokens=16)
     weights = wl.make_weights(w.model, 13)

@@ -176,9 +176,11 @@ def test_config1_end_to_end(B, path):
     m.close()
 
 
-@pytest.mark.parametrize("mode", [0, 1])
-def test_tiny_gqa_ragged_prompts(B, mode):
-    """GQA (r = 4), head_dim 64, prompts whose lengths are not page multiples, Gumbel sampling."""
+@pytest.mark.parametrize("mode,step_kernel", [(0, 0), (1, 0), (0, 1), (1, 1)])
+def test_tiny_gqa_ragged_prompts(B, monkeypatch, mode, step_kernel):
+    """GQA (r = 4), head_dim 64, prompts whose lengths are not page multiples, Gumbel sampling; per-layer kernels and
+    the persistent decode-step kernel."""
+    monkeypatch.setenv("SAGC_STEP", str(step_kernel))
     w = wl.tiny_variant(1, model_n_q_heads=8, model_n_kv_heads=2, model_head_dim=64, model_d_model=256,
                         model_d_ff=768, model_n_layers=3, model_vocab=2048, model_page_tokens=16)
     weights = wl.make_weights(w.model, 1)
@@ -285,18 +287,20 @@ def _sampled_parity(B, cfg, n_prompts, P, G, max_new, fl, path, n_dump_seq=3):
 @pytest.mark.parametrize("variant", ["step_kernel", "per_layer_kernels", "register_hmma"])
 def test_config2_truncated(B, monkeypatch, variant):
     """0.5B shape: 2 prompts x 256 x G=8 (16 live rows, then fewer) through the three decode paths that exist:
-    the persistent decode-step kernel (default), the per-layer tcgen05 kernels (SAGC_STEP=0) and the
+    the per-layer tcgen05 kernels (default), the persistent decode-step kernel (SAGC_STEP=1) and the
     register-HMMA kernels (SAGC_TC=0: the path of shapes that are not multiples of 128)."""
-    if variant == "per_layer_kernels":
-        monkeypatch.setenv("SAGC_STEP", "0")
+    if variant == "step_kernel":
+        monkeypatch.setenv("SAGC_STEP", "1")
     if variant == "register_hmma":
         monkeypatch.setenv("SAGC_TC", "0")
     fl = np.array([3, 14, 14, 2, 14, 9, 5, 14, 14, 1, 14, 7, 14, 14, 4, 14], dtype=np.int32)
     _sampled_parity(B, 2, 2, 256, 8, 14, fl, 0)
 
 
-def test_config3_truncated(B):
+@pytest.mark.parametrize("step_kernel", [0, 1])
+def test_config3_truncated(B, monkeypatch, step_kernel):
     """1.5B shape (head_dim 128, r = 6, DAPO config): 1 prompt x 96 tokens (ragged vs the 64-token page) x G=16."""
+    monkeypatch.setenv("SAGC_STEP", str(step_kernel))
     fl = np.array([10, 3, 10, 10, 1, 10, 7, 10, 10, 10, 5, 10, 10, 2, 10, 10], dtype=np.int32)
     _sampled_parity(B, 3, 1, 96, 16, 10, fl, 0, n_dump_seq=2)
 
