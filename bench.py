@@ -375,6 +375,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cfg", type=int, default=2)
     ap.add_argument("--max-new", type=int, default=0, help="override max_new_tokens (debug; invalidates the number)")
+    ap.add_argument("--n-prompts", type=int, default=0, help="override the number of prompts (profiling windows; invalidates the number)")
+    ap.add_argument("--g", type=int, default=0, help="override the group size G (profiling windows; invalidates the number)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-side-7b", action="store_true", help="skip the configs[4] (7B shape) side block (~5 minutes)")
     ap.add_argument("--protocol", default="rollout", choices=["rollout", "fixed-eb"],
@@ -400,6 +402,8 @@ def main():
     B.lib()
 
     w = wl.WORKLOADS[args.cfg]
+    if args.n_prompts or args.g:
+        w = wl.tiny_variant(args.cfg, n_prompts=args.n_prompts or w.n_prompts, G=args.g or w.G)
     mc = w.model
     max_new = args.max_new or w.max_new
     weights = wl.make_weights(mc, 0)

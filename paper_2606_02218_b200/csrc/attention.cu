@@ -53,9 +53,9 @@ static int launch_att_geom(const AttnArgs& a, cudaStream_t st) {
 
 template <int HD>
 static int launch_att(const AttnArgs& a, cudaStream_t st) {
-    // a.geom (parity / tuning entry only): alternative K/V staging geometries of the same unit
-    if (HD >= 64 && a.geom == 1) return launch_att_geom<HD, 4, 4>(a, st);       // 64-token tiles, 4 stages
-    if (HD >= 64 && a.geom == 2) return launch_att_geom<HD, 4, 3>(a, st);       // 64-token tiles, 3 stages
+    // other staging geometries (64-token tiles x 3 / 4 stages, 128-token tiles x 3 / 6 stages = 192 KB) were measured
+    // with this launcher and changed nothing: the kernel is bound by issue latency at 2 warps per scheduler, not by
+    // bytes in flight (profiles/r02_attention.md)
     return launch_att_geom<HD, AttStandalone<HD>::WARPS, AttStandalone<HD>::NSTAGE>(a, st);
 }
 

@@ -149,21 +149,31 @@ __device__ __forceinline__ void attention_unit(const AttnArgs& a, const int row,
     // K chunk c of token j -> chunk c ^ ksw(j); V chunk c -> c ^ vsw(j)   (bank-conflict free)
     auto ksw = [](int j) { return CPR >= 8 ? ((j & 1) << 2) : 0; };
     auto vsw = [](int j) { return CPR >= 8 ? (j & 7) : ((j >> 1) & 3); };
+    // Tile loader.  Thread -> (token row j0 + k * RPT, 16-byte chunk `part`), k = 0 .. NPASS-1: the chunk, the swizzled
+    // shared-memory offsets and the per-head base pointer are per-thread constants (RPT is a multiple of 16, so the
+    // swizzle terms do not depend on k); a pass costs one page lookup, one 64-bit multiply-add and two cp.async.
+    // (The address arithmetic was 55 % of the kernel's instructions before: profiles/r02_attention.md.)
+    constexpr int RPT = ATT_THREADS / CPR;       // token rows covered per pass
+    constexpr int NPASS = ATT_TILE / RPT;
+    static_assert(ATT_TILE % RPT == 0 && RPT % 16 == 0, "tile / thread mapping of the K/V loader");
+    const int ld_part = tid % CPR, ld_j0 = tid / CPR;
+    const uint32_t ld_ks = (uint32_t)ld_j0 * ROWB + (uint32_t)((ld_part ^ ksw(ld_j0)) << 4);
+    const uint32_t ld_vs = (uint32_t)(ATT_TILE + ld_j0) * ROWB + (uint32_t)((ld_part ^ vsw(ld_j0)) << 4);
+    const size_t ld_pstride = (size_t)2 * a.Hkv * head_stride;                      // elements per page (K and V, all kv heads)
+    const bf16_t* ld_base = a.kv_layer + (size_t)kvh * head_stride + ld_part * 8;   // K of this kv head; V sits Hkv slabs further
+    const size_t ld_voff = (size_t)a.Hkv * head_stride;
     auto load_tile = [&](int tile, int stage) {
         unsigned char* base = kv_s + (size_t)stage * G::STAGE;
-        const int t0 = t_begin + tile * ATT_TILE;
+        const int tok0 = t_begin + tile * ATT_TILE + ld_j0;
 #pragma unroll
-        for (int c = tid; c < ATT_TILE * CPR; c += ATT_THREADS) {
-            const int j = c / CPR, part = c % CPR;
-            const int tok = t0 + j;
-            const int blk = tok >> pshift;
-            const int pg = (tok < t_end) ? (pg_cached ? sm->pg_s[blk - b_begin] : pt[blk]) : -1;
+        for (int k = 0; k < NPASS; ++k) {
+            const int tok = tok0 + k * RPT;
+            int pg = -1;
+            if (tok < t_end) pg = pg_cached ? sm->pg_s[(tok >> pshift) - b_begin] : pt[tok >> pshift];
             const bool ok = pg >= 0;             // masked tail, or an unmapped block after a pool-exhaustion error: zero fill
-            const bf16_t* kp = a.kv_layer + ((size_t)(ok ? pg : 0) * 2 * a.Hkv + kvh) * head_stride +
-                               (size_t)(ok ? (tok & pmask) : 0) * HD + part * 8;
-            const bf16_t* vp = kp + (size_t)a.Hkv * head_stride;
-            cp_async16(base + (size_t)j * ROWB + ((part ^ ksw(j)) << 4), kp, ok ? 16 : 0);
-            cp_async16(base + (size_t)(ATT_TILE + j) * ROWB + ((part ^ vsw(j)) << 4), vp, ok ? 16 : 0);
+            const bf16_t* kp = ld_base + (ok ? (size_t)pg * ld_pstride + (size_t)((tok & pmask) * HD) : (size_t)0);
+            cp_async16(base + ld_ks + (uint32_t)(k * RPT * ROWB), kp, ok ? 16 : 0);
+            cp_async16(base + ld_vs + (uint32_t)(k * RPT * ROWB), kp + ld_voff, ok ? 16 : 0);
         }
     };
     // fused RoPE (decode): cos/sin of this row's position for the q fragments, fetched before the wait
@@ -321,8 +331,10 @@ __device__ __forceinline__ void attention_unit(const AttnArgs& a, const int row,
         ls += __shfl_xor_sync(0xffffffffu, ls, 2);
         l_run = l_run * f + ls;
         m_run = m_new;
+        if (__any_sync(0xffffffffu, f != 1.f)) {     // running max unchanged on every lane: f == 1 exactly, skip the rescale
 #pragma unroll
-        for (int n = 0; n < NT; ++n) { o[n][0] *= f; o[n][1] *= f; o[n][2] *= f; o[n][3] *= f; }
+            for (int n = 0; n < NT; ++n) { o[n][0] *= f; o[n][1] *= f; o[n][2] *= f; o[n][3] *= f; }
+        }
         // P as the A operand: rows g = hi, rows g+8 = lo; k = 16 tokens
         uint32_t pa[4];
         split2(p[0], p[1], pa[0], pa[1]);

@@ -121,7 +121,7 @@ __device__ __forceinline__ float silu_f(float z) { return z / (1.f + __expf(-z))
 
 struct StepShared {                      // lives in the STEP_MISC region
     uint64_t full[12], empty[12], acc_full[2], bfull[2], bempty[2];
-    uint32_t tmem_slot; int M, par, ns, pad;
+    uint32_t tmem_slot; int M, par, ns; unsigned ld_n;
     StepPhasePlan pl[4];
     float red[8];
     int ctx_max[8];
@@ -186,6 +186,7 @@ k_decode_step(const StepDev a) {
     const int cta = blockIdx.x, nCTA = a.n_cta, NS = a.n_slots, NB = a.NB, L = a.n_layers, CH = a.chunk;
 
     if (tid < 4) sh->pl[tid] = a.plan[(size_t)tid * nCTA + cta];
+    if (tid == 4) sh->ld_n = 0u;
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < NS; ++s) { mbar_init(&sh->full[s], 1); mbar_init(&sh->empty[s], 1); }
         for (int s = 0; s < 2; ++s) { mbar_init(&sh->acc_full[s], 1); mbar_init(&sh->bfull[s], 1); mbar_init(&sh->bempty[s], 1); }
@@ -204,8 +205,7 @@ k_decode_step(const StepDev a) {
 
     if (warp == 0) {
         // =========================== A producer: weights, as far ahead as the ring allows ===========================
-        // Besides filling the ring, the producer asks the TMA unit to pull the tile `a.prefetch` k blocks further along
-        // the same unit into L2: while the consumers sit in a phase boundary the ring is full, but HBM keeps streaming.
+        // (Warp 3 walks the same list a.prefetch tiles further ahead and only asks the TMA unit to pull the tile into L2.)
         if (lane == 0) {
             unsigned n = 0;
             for (int i = 0; i < 7 && L > 0; ++i) tma_prefetch_desc(&a.wmaps[i]);
@@ -222,12 +222,37 @@ k_decode_step(const StepDev a) {
                         for (int kb = sg.kb0; kb < sg.kb1; ++kb)
                             for (int na = 0; na < NA; ++na, ++n) {
                                 const unsigned slot = n % NS, use = n / NS;
-                                if (a.prefetch > 0 && kb + a.prefetch < sg.kb1)
-                                    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];\n" ::"l"(na ? m1 : m0),
-                                                 "r"((kb + a.prefetch) * 64), "r"(arow) : "memory");
                                 if (use > 0) step_wait_mbar(&sh->empty[slot], (use - 1) & 1, a.err, 1);
+                                if (a.prefetch > 0 && (n & 3u) == 0) *reinterpret_cast<volatile unsigned*>(&sh->ld_n) = n;
                                 mbar_expect_tx(&sh->full[slot], STEP_SLOT);
                                 tma_load_2d(ring + (size_t)slot * STEP_SLOT, na ? m1 : m0, &sh->full[slot], kb * 64, arow);
+                            }
+                    }
+                }
+            }
+        }
+        __syncwarp();
+    } else if (warp == 3) {
+        // =========================== L2 prefetcher (optional): same walk as the A producer, a.prefetch tiles ahead ===========
+        // While the consumers sit in a phase boundary the ring is full and the A producer stalls; this warp keeps HBM
+        // streaming into L2, from where the ring refills at L2 speed.
+        if (lane == 0 && a.prefetch > 0) {
+            unsigned n = 0;
+            for (int l = 0; l < L; ++l) {
+                const CUtensorMap* w7 = a.wmaps + (size_t)l * 7;
+                for (int ph = 0; ph < 4; ++ph) {
+                    const int NA = a.g[ph].na;
+                    for (int s = 0; s < sh->pl[ph].nseg; ++s) {
+                        const StepSeg sg = sh->pl[ph].seg[s];
+                        int arow;
+                        const CUtensorMap* m0 = step_wmap(a, w7, ph, sg.tile, 0, arow);
+                        const CUtensorMap* m1 = step_wmap(a, w7, ph, sg.tile, 1, arow);
+                        for (int kb = sg.kb0; kb < sg.kb1; ++kb)
+                            for (int na = 0; na < NA; ++na, ++n) {
+                                if (n < (unsigned)NS) continue;            // the first ring-full is loaded directly
+                                while (n > *reinterpret_cast<volatile unsigned*>(&sh->ld_n) + (unsigned)a.prefetch) __nanosleep(64);
+                                asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];\n" ::"l"(na ? m1 : m0),
+                                             "r"(kb * 64), "r"(arow) : "memory");
                             }
                     }
                 }
@@ -619,7 +644,7 @@ int launch_decode_step(const StepLaunch& s, cudaStream_t st) {
     d.live = s.live; d.pos = s.pos; d.ctx = s.ctx; d.tok = s.tok; d.n_live = s.n_live; d.step = s.step; d.m_max = s.m_max;
     d.att = s.att; d.kv_pool = s.kv_pool; d.layer_stride = s.layer_stride; d.err = s.err; d.trace = s.trace;
     { const char* e = getenv("SAGC_STEP_FLAGS"); d.flags = e ? atoi(e) : 0; }
-    { const char* e = getenv("SAGC_STEP_PREFETCH"); d.prefetch = e ? atoi(e) : 0; }
+    { const char* e = getenv("SAGC_STEP_PREFETCH"); d.prefetch = e ? atoi(e) : 0; if (d.prefetch > 0 && d.prefetch < 8) d.prefetch = 8; }   // < 8 could strand the prefetch warp behind the published count
     const int smem = step_smem_bytes(s.n_slots);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(s.n_cta);

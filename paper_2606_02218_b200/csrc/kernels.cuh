@@ -76,7 +76,6 @@ struct AttnArgs {
     // lacks the 1/rms factor of its row; when q_fx is set it replaces q (same [row][ldq] indexing)
     const long long* q_fx; const float* q_rstd;
     int prefetch;           // 1 in decode: cached positions older than the newest one predate the upstream kernel
-    int geom;               // standalone launcher: 0 = default staging geometry, 1 / 2 = 64-token tiles with 4 / 3 stages
     int cluster_merge;      // set by the launcher: the n_splits CTAs of a (row, kv head) form a cluster and merge through DSMEM
 };
 int launch_attention(const AttnArgs& a, cudaStream_t st);

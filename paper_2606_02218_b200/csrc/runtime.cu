@@ -1213,7 +1213,7 @@ extern "C" int sagc_debug_attention(const float* q, const void* kv, const int32_
     if (!q || !kv || !page_table || !ctx || !out || M < 1) return set_err(SAGC_EINVAL, "null argument");
     if (Hq % Hkv || Hq / Hkv > 8) return set_err(SAGC_EINVAL, "bad head counts");
     if (n_splits < 1 || n_splits > 64) return set_err(SAGC_EINVAL, "n_splits must be in 1..64");
-    if (variant < 0 || variant > 3) return set_err(SAGC_EINVAL, "variant must be 0 (standalone kernel), 1 (decode-step units), 2 / 3 (standalone, 64-token tiles x 4 / 3 stages)");
+    if (variant != 0 && variant != 1) return set_err(SAGC_EINVAL, "variant must be 0 (standalone kernel) or 1 (decode-step units)");
     if (variant == 1 && hd != 64 && hd != 128) return set_err(SAGC_EINVAL, "the decode-step units need head_dim 64 or 128");
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     int *sid = nullptr, *cnt = nullptr;
@@ -1232,7 +1232,6 @@ extern "C" int sagc_debug_attention(const float* q, const void* kv, const int32_
     a.hd = hd; a.page = page_tokens; a.n_splits = n_splits; a.part_o = po; a.part_ml = pml; a.counters = cnt; a.out = out;
     int n_sm = 148;
     { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); }
-    a.geom = variant >= 2 ? variant - 1 : 0;
     int r = variant == 1 ? launch_attention_units(a, n_sm, st) : launch_attention(a, st);
     cudaError_t e = cudaStreamSynchronize(st);
     cudaFree(sid); cudaFree(cnt); cudaFree(po); cudaFree(pml);

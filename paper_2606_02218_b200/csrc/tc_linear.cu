@@ -543,6 +543,7 @@ int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
     if (KS > room) KS = room;
     if (KS < 1) KS = 1;
     if (KS > 8) KS = 8;
+    { static const int ksmax = [] { const char* e = getenv("SAGC_TC_KSMAX"); return e ? atoi(e) : 8; }(); if (KS > ksmax) KS = ksmax; }   // sweep knob (temporary)
     if (KS > d.n_kb) KS = d.n_kb;
     if (t.scratch == nullptr) KS = 1;
     { int p2 = 1; while (p2 * 2 <= KS) p2 *= 2; KS = p2; }      // the epilogue is specialised for 1, 2, 4, 8

@@ -101,12 +101,14 @@ def test_philox_draws_bit_exact(B, seed, sid, t, v0, n):
 
 # ---------------------------------------------------------------------------- a6, a8-a11
 @pytest.mark.parametrize("N,K", [(64, 128), (128, 64), (896, 896), (896, 4864), (1152, 896), (2048, 1536), (20000 // 16 * 16, 256), (19968, 256)])
-@pytest.mark.parametrize("M", [1, 3, 8, 13, 17, 40, 64, 70, 131, 300])
+@pytest.mark.parametrize("M", [1, 3, 8, 13, 17, 40, 64, 70, 131, 300, 512, 2048])
 @pytest.mark.parametrize("path", [1, 2, 3])
 def test_linear_vs_fp64(B, N, K, M, path):
     """path 1: fp32 GEMV; 2: tcgen05 (falls back to mma.sync when N % 128 or K % 64); 3: mma.sync."""
     if path == 1 and M > 13:
         pytest.skip("GEMV path is the tail path")
+    if M > 300 and (path != 2 or N > 4096):
+        pytest.skip("prefill-sized row counts: tcgen05 path, projection-sized outputs")
     rng = np.random.default_rng(N * 31 + K * 7 + M)
     Wb = wl.f32_to_bf16_bits((0.02 * rng.standard_normal((N, K))).astype(np.float32))
     x = rng.standard_normal((M, K)).astype(np.float32)
