@@ -542,8 +542,7 @@ int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
     if ((size_t)2 * g_num_sms * 2 * 128 * 128 > TC_SCRATCH_FLOATS) return -1;      // split-K scratch is sized for 296 CTAs
     if (KS > room) KS = room;
     if (KS < 1) KS = 1;
-    if (KS > 8) KS = 8;
-    { static const int ksmax = [] { const char* e = getenv("SAGC_TC_KSMAX"); return e ? atoi(e) : 8; }(); if (KS > ksmax) KS = ksmax; }   // sweep knob (temporary)
+    if (KS > 8) KS = 8;     // cap re-swept in round 2 (decode step, cap 8 / 4 / 2): 1.5B 1.42 / - / 1.80 ms, 7B 3.35 / 3.60 / 5.06 ms
     if (KS > d.n_kb) KS = d.n_kb;
     if (t.scratch == nullptr) KS = 1;
     { int p2 = 1; while (p2 * 2 <= KS) p2 *= 2; KS = p2; }      // the epilogue is specialised for 1, 2, 4, 8
