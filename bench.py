@@ -248,8 +248,9 @@ def new_acc():
             "prefill_ms": 0.0, "prefill_flops": 0.0, "decode_ms": 0.0}
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch from `ncu --set full` (profiles/r02_ncu_top_kernels.md), by shape
-NCU_TRAFFIC = {}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE decode step (the sum over the step's kernels, <= 8 live rows) from the
+# `ncu --set full` captures in profiles/r02_ncu_top_kernels.md, by config: within 2 % of the step's algorithmic bytes
+NCU_TRAFFIC = {2: 1.045e9, 4: 1.448e10, 5: 1.448e10}
 
 
 def kernel_parts(model, B, w, d_prompts, offs, fl, max_new, mode, peak):
@@ -483,16 +484,19 @@ def main():
             "clocks": clocks, "gpu_launches": acc["launches"],
             "e2e": {"value": world * e2e_tok / e2e_ms * 1e3, "unit": UNIT, "h2d_bytes_per_step": int(prompts.nbytes + fl.nbytes),
                     "d2h_bytes_per_step": int(nseq * max_new * 4 + nseq * 4 + w.n_prompts * 16)},
-            # the dominant kernel: the layer stack of a decode step (one persistent launch per step while <= 64 rows are live)
-            "roofline": {"bound": "hbm", "achieved": ls["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": ls["frac"],
-                         "traffic": NCU_TRAFFIC.get((args.cfg, "layer_stack")), "peak_source": peak_src,
-                         "kernel": ls["kernel"], "share_of_decode_step": ls["share_of_step"],
-                         "what": "layer-stack launch of every decode step of one rollout, timed alone with CUDA events on the launching stream "
-                                 "(SAGC_FLAG_TIME_KERNELS): algorithmic bytes (layer weights once + prefix KV once per live group + suffix KV + "
-                                 "KV written) / device time",
-                         "frac_of_8tbs": ls["achieved_gbs"] / 8000.0},
-            "roofline_all_decode": {"achieved": achieved, "frac": achieved / peak, "frac_of_8tbs": achieved / 8000.0,
-                                    "what": "every kernel of every decode step of the timed rollouts (graph launches): algorithmic bytes / device time"},
+            # Headline roofline = EVERY kernel of every decode step of the timed rollouts (CUDA-graph launches of the step's
+            # kernel chain), not the best part of it: algorithmic bytes of all decode steps / device time of all decode steps.
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": NCU_TRAFFIC.get(args.cfg), "peak_source": peak_src,
+                         "kernel": "one decode step = " + ls["kernel"] + "; then LM head + sampler, advance",
+                         "what": "all decode steps of the timed rollouts: algorithmic bytes (layer + LM-head weights once per step + prefix KV once "
+                                 "per live group + suffix KV + KV written) / device time between the step-boundary events of the rollout stream",
+                         "frac_of_8tbs": achieved / 8000.0},
+            # the layer stack of the step timed alone (direct launches bracketed by events, SAGC_FLAG_TIME_KERNELS), with its
+            # share of the step; in_graph_estimate = the same bytes over the layer stack's share of the graph-run step time
+            "roofline_layer_stack": {"achieved": ls["achieved_gbs"], "frac": ls["frac"], "share_of_decode_step": ls["share_of_step"],
+                                     "kernel": ls["kernel"], "bytes_per_step": ls["bytes_per_step"],
+                                     "in_graph_estimate_gbs": (ls["bytes_per_step"] * parts["steps_measured"]) / max(ls["share_of_step"] * dec_ms / args.steps, 1e-9) / 1e6},
             "phases": phase_table(acc, args.steps, peak, mc, tf_sus), "kernel_roofline": parts,
             "prefill": {"ms": acc["prefill_ms"] / args.steps, "tflops": acc["prefill_flops"] / acc["prefill_ms"] / 1e9 if acc["prefill_ms"] else None}}
     if not args.no_cpu_baseline:

@@ -227,6 +227,23 @@ int sagc_debug_attention(const float* q, const void* kv, const int32_t* page_tab
                          int32_t M, int32_t Hq, int32_t Hkv, int32_t hd, int32_t page_tokens,
                          int32_t max_blocks, int32_t n_splits, int32_t variant, float* out, void* stream);
 
+/* The same split-K attention (step a7) for callers that may not allocate: code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc.  Arguments as sagc_debug_attention (all DEVICE pointers, caller
+ * owned; out dev float [M][Hq][hd]); always the one-CTA-per-(row, kv head, split) kernel with the last-arriver
+ * merge through scratch memory.  That scratch -- arrival counters, the live list, the (max, sum) pairs and the
+ * partial outputs, 4 * (M*Hkv + M + M*Hq*n_splits*(2 + hd)) bytes plus 256-byte rounding of each part -- lives in
+ * ONE static device array of SAGC_NOALLOC_SCRATCH_BYTES that every GPU which loads the library holds until exit.
+ *   - calls no cudaMalloc / cudaFree / allocating library routine; enqueues two kernels on `stream` and returns
+ *     WITHOUT synchronising (errors of the kernels themselves surface at the caller's next synchronisation);
+ *   - SAGC_EINVAL with a message naming the sizes when the scratch need exceeds SAGC_NOALLOC_SCRATCH_BYTES, or on
+ *     bad shapes; SAGC_ECUDA when the array's address cannot be taken or a launch fails;
+ *   - every call shares the array (counters and live list are re-initialised at the start of each call): calls
+ *     that OVERLAP on the GPU -- different streams without an event between them -- race and give garbage. */
+#define SAGC_NOALLOC_SCRATCH_BYTES (8u << 20)
+int sagc_attention_noalloc(const float* q, const void* kv, const int32_t* page_table, const int32_t* ctx,
+                           int32_t M, int32_t Hq, int32_t Hkv, int32_t hd, int32_t page_tokens,
+                           int32_t max_blocks, int32_t n_splits, float* out, void* stream);
+
 const char* sagc_last_error(void);
 const char* sagc_version(void);
 

@@ -27,7 +27,7 @@ EXPORTS = [
     "sagc_model_create", "sagc_model_destroy", "sagc_rollout_group", "sagc_rollout_group_host", "sagc_score_tokens",
     "sagc_group_advantage", "sagc_length_stats", "sagc_debug_page_table", "sagc_debug_free_stack",
     "sagc_debug_alloc_log", "sagc_debug_retire_log", "sagc_debug_peak_pages", "sagc_debug_philox",
-    "sagc_debug_linear", "sagc_debug_lm_sample", "sagc_debug_attention", "sagc_debug_step_trace", "sagc_last_error", "sagc_version",
+    "sagc_debug_linear", "sagc_debug_lm_sample", "sagc_debug_attention", "sagc_attention_noalloc", "sagc_debug_step_trace", "sagc_last_error", "sagc_version",
 ]
 
 
@@ -100,6 +100,8 @@ def lib():
         L.sagc_debug_attention.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32,
                                            C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p,
                                            C.c_void_p]
+        L.sagc_attention_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32,
+                                             C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         L.sagc_debug_step_trace.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_int32, C.POINTER(C.c_int32)]
         _lib = L
     return _lib
@@ -354,4 +356,21 @@ def debug_attention(q: torch.Tensor, kv_bits: torch.Tensor, page_table: torch.Te
     _check(lib().sagc_debug_attention(q.data_ptr(), kv_bits.data_ptr(), page_table.data_ptr(), ctx.data_ptr(), M, Hq,
                                       Hkv, hd, page_tokens, page_table.shape[1], n_splits, variant, out.data_ptr(),
                                       _stream()))
+    return out
+
+
+NOALLOC_SCRATCH_BYTES = 8 << 20
+
+
+def attention_noalloc(q: torch.Tensor, kv_bits: torch.Tensor, page_table: torch.Tensor, ctx: torch.Tensor, out: torch.Tensor,
+                      Hq: int, Hkv: int, hd: int, page_tokens: int, n_splits: int = 4) -> torch.Tensor:
+    """sagc_attention_noalloc: shapes as `debug_attention`, but `out` (float32 [M][Hq][hd]) is the caller's and the
+    split-K scratch is the library's static device array (<= NOALLOC_SCRATCH_BYTES, else SagcError).  Nothing is
+    allocated and the stream is not synchronised; calls that overlap on the GPU race on the shared scratch."""
+    _require_cuda()
+    M = q.shape[0]
+    if out.dtype != torch.float32 or out.numel() != M * Hq * hd or not out.is_contiguous():
+        raise ValueError("out must be a contiguous float32 [M][Hq][hd] tensor")
+    _check(lib().sagc_attention_noalloc(q.data_ptr(), kv_bits.data_ptr(), page_table.data_ptr(), ctx.data_ptr(), M, Hq,
+                                        Hkv, hd, page_tokens, page_table.shape[1], n_splits, out.data_ptr(), _stream()))
     return out

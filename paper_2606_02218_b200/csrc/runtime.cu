@@ -43,6 +43,7 @@ static int set_err(int code, const char* fmt, ...) {
     return code;
 }
 extern "C" const char* sagc_last_error(void) { return g_err; }
+namespace sagc { int api_set_error(int code, const char* msg) { return set_err(code, "%s", msg); } }   // for entry points in other files
 extern "C" const char* sagc_version(void) { return "sagc-rollout 0.1 (sm_100a)"; }
 
 #define CU(x)                                                                                   \
