@@ -222,6 +222,8 @@ int sagc_debug_lm_sample(const void* W, const float* x, int32_t M, int32_t V, in
  *   variant 0: the standalone kernel (one CTA per unit; 2..8 splits merge inside a cluster through DSMEM,
  *              more through the L2 scratch);  variant 1: the units as the persistent decode-step kernel runs
  *              them (one CTA per SM looping over units, last-arriver merge; head_dim 64 / 128 only).
+ *   variant 2: the tcgen05 kernel of the decode steps (TMA-staged pages, S and O in tensor memory; head_dim 64 / 128,
+ *              pages of 8 .. 128 tokens; last-arriver merge for any n_splits).
  *   Synchronises the stream.  SAGC_EINVAL on bad shapes. */
 int sagc_debug_attention(const float* q, const void* kv, const int32_t* page_table, const int32_t* ctx,
                          int32_t M, int32_t Hq, int32_t Hkv, int32_t hd, int32_t page_tokens,

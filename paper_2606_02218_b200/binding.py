@@ -349,7 +349,7 @@ def debug_lm_sample(W_bits: torch.Tensor, x: torch.Tensor, sids: torch.Tensor, t
 def debug_attention(q: torch.Tensor, kv_bits: torch.Tensor, page_table: torch.Tensor, ctx: torch.Tensor, Hq: int,
                     Hkv: int, hd: int, page_tokens: int, n_splits: int = 4, variant: int = 0) -> torch.Tensor:
     """q float32 [M][Hq][hd]; kv_bits int16 [n_pages][2][Hkv][page][hd]; page_table int32 [M][max_blocks].
-    variant 0 = standalone kernel, 1 = the units of the persistent decode-step kernel."""
+    variant 0 = standalone kernel, 1 = the units of the persistent decode-step kernel, 2 = the tcgen05 decode kernel."""
     _require_cuda()
     M = q.shape[0]
     out = torch.empty((M, Hq, hd), dtype=torch.float32, device=q.device)

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsagc.so")
-SOURCES = ["linear.cu", "tc_linear.cu", "attention.cu", "attention_noalloc.cu", "decode_step.cu", "elementwise.cu", "sampler.cu", "paging.cu", "groupstats.cu", "runtime.cu"]
+SOURCES = ["linear.cu", "tc_linear.cu", "attention.cu", "attention_noalloc.cu", "attention_tc.cu", "decode_step.cu", "elementwise.cu", "sampler.cu", "paging.cu", "groupstats.cu", "runtime.cu"]
 HEADERS = ["common.cuh", "kernels.cuh", "tc_ptx.cuh", "attention_body.cuh", os.path.join("..", "..", "include", "sagc.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]

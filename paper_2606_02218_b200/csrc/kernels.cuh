@@ -80,6 +80,12 @@ struct AttnArgs {
 };
 int launch_attention(const AttnArgs& a, cudaStream_t st);
 
+// tcgen05 decode attention (attention_tc.cu): head_dim 64 / 128, pages of 8 .. 128 tokens; split merge through the L2 scratch
+struct TcMap;
+bool attention_tc_supports(int hd, int page, int r);
+int attention_tc_make_map(TcMap* out, const void* kv_layer, long long n_pages, int Hkv, int page, int hd);
+int launch_attention_tc(const AttnArgs& a, const TcMap* kvmap, int stages, cudaStream_t st);
+
 // Sampler over fp32 logits.  Step a3 / a12.
 static constexpr int SMP_CHUNKS = 32;
 struct SampleArgs {

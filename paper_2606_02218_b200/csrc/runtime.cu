@@ -106,6 +106,8 @@ struct sagc_model {
     float* tc_scratch;
     int ssq_ld, d_tiles;
     std::vector<TcMap> wmaps;                  // per layer: q k v o g u d ; last = lm_head
+    std::vector<TcMap> kvmaps;                 // per layer: the KV pool as a 2-D tensor (tcgen05 decode attention)
+    int att_tc, att_tc_stages;                 // SAGC_ATT_TC (default 1): decode attention on tcgen05; ring depth (0 = deepest)
     TcMap amaps[3][4];                         // {xs, att_s, act_s} x UMMA N {32, 64, 128, 256}
     // persistent decode-step kernel (decode_step.cu): static work plan, device copies of the per-layer tables, counters
     bool step_ok; int n_sm, step_slots, gbar_n, tcnt_n, tiles_per_layer;
@@ -208,6 +210,21 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     m->step_ok = false; m->n_sm = 0; m->step_trace = nullptr;
 
     DA(m->kv_pool, m->layer_stride * (size_t)(L > 0 ? L : 1));
+    // finite everywhere: a masked position of a partially filled page meets p = 0 in the tcgen05 attention (0 * NaN would not be 0)
+    if (cudaMemset(m->kv_pool, 0, m->layer_stride * (size_t)(L > 0 ? L : 1) * sizeof(bf16_t)) != cudaSuccess) {
+        sagc_model_destroy(m);
+        return set_err(SAGC_ECUDA, "cudaMemset of the KV pool failed");
+    }
+    m->att_tc = env_int("SAGC_ATT_TC", 1) && attention_tc_supports(c.head_dim, c.page_tokens, c.n_q_heads / c.n_kv_heads);
+    m->att_tc_stages = env_int("SAGC_ATT_TC_STAGES", 0);
+    if (m->att_tc) {
+        m->kvmaps.resize(L > 0 ? L : 1);
+        for (int l = 0; l < L; ++l)
+            if (attention_tc_make_map(&m->kvmaps[l], m->kv_pool + (size_t)l * m->layer_stride, c.n_pages, c.n_kv_heads, c.page_tokens, c.head_dim) != 0) {
+                m->att_tc = 0;      // no driver entry point for tensor maps: the register-HMMA unit serves decode too
+                break;
+            }
+    }
     // RoPE table: angle = pos * theta^(-2i/hd) and cos/sin in fp64 on the host, stored as fp32
     {
         const int half = c.head_dim / 2;
@@ -441,7 +458,10 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cuda
         aa.n_splits = n_splits; aa.part_o = m->part_o; aa.part_ml = m->part_ml; aa.counters = m->counters;
         aa.out = m->att; aa.prefetch = (rs.m_dev != nullptr) ? 1 : 0; aa.out_split = m->att_s; aa.ld_split = qd;
         aa.fuse_rope = fuse_att ? 1 : 0; aa.rope_cs = m->rope_cs; aa.row_pos = rs.pos; aa.kv_layer_w = kv_layer;
-        if (!(skip & 1)) LAUNCH(launch_attention(aa, st));
+        if (!(skip & 1)) {
+            if (fuse_att && m->att_tc) LAUNCH(launch_attention_tc(aa, &m->kvmaps[l], m->att_tc_stages, st));
+            else LAUNCH(launch_attention(aa, st));
+        }
 
         TcLinearArgs o = {};
         o.a[0] = &w7[3]; o.seg_rows[0] = c.d_model; o.b = &m->amaps[1][nbi]; o.K = qd; o.N = c.d_model;
@@ -523,6 +543,17 @@ static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
     while (s * 2 <= want) s *= 2;
     const int smax = 8;                       // <= 8 splits merge inside a cluster (attention.cu)
     if (s > smax) s = smax;
+    if (m->att_tc && m->cfg.head_dim >= 64) {
+        // tcgen05 decode attention: one CTA per SM (the K/V ring fills shared memory), >= 2 tiles of 128 tokens per
+        // split, partials merged through L2 by the last arriver (no cluster limit)
+        int w2 = sagc::g_num_sms / ctas;
+        const int cap2 = ctx_bound / 256;
+        if (w2 > cap2) w2 = cap2;
+        if (w2 > 32) w2 = 32;
+        if (w2 > m->max_splits) w2 = m->max_splits;
+        s = 1;
+        while (s * 2 <= w2) s *= 2;
+    }
     return s;
 }
 
@@ -1214,7 +1245,8 @@ extern "C" int sagc_debug_attention(const float* q, const void* kv, const int32_
     if (!q || !kv || !page_table || !ctx || !out || M < 1) return set_err(SAGC_EINVAL, "null argument");
     if (Hq % Hkv || Hq / Hkv > 8) return set_err(SAGC_EINVAL, "bad head counts");
     if (n_splits < 1 || n_splits > 64) return set_err(SAGC_EINVAL, "n_splits must be in 1..64");
-    if (variant != 0 && variant != 1) return set_err(SAGC_EINVAL, "variant must be 0 (standalone kernel) or 1 (decode-step units)");
+    if (variant < 0 || variant > 2) return set_err(SAGC_EINVAL, "variant must be 0 (standalone kernel), 1 (decode-step units) or 2 (tcgen05 kernel)");
+    if (variant == 2 && !attention_tc_supports(hd, page_tokens, Hq / Hkv)) return set_err(SAGC_EINVAL, "the tcgen05 kernel needs head_dim 64 / 128 and pages of 8 .. 128 tokens");
     if (variant == 1 && hd != 64 && hd != 128) return set_err(SAGC_EINVAL, "the decode-step units need head_dim 64 or 128");
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     int *sid = nullptr, *cnt = nullptr;
@@ -1233,7 +1265,23 @@ extern "C" int sagc_debug_attention(const float* q, const void* kv, const int32_
     a.hd = hd; a.page = page_tokens; a.n_splits = n_splits; a.part_o = po; a.part_ml = pml; a.counters = cnt; a.out = out;
     int n_sm = 148;
     { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); }
-    int r = variant == 1 ? launch_attention_units(a, n_sm, st) : launch_attention(a, st);
+    int r;
+    if (variant == 2) {
+        // the pool's extent is not an argument: take it from the largest page id in the caller's table
+        std::vector<int> pt_h((size_t)M * max_blocks);
+        CU(cudaMemcpyAsync(pt_h.data(), page_table, pt_h.size() * sizeof(int), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        long long n_pages = 1;
+        for (int v : pt_h) if ((long long)v + 1 > n_pages) n_pages = (long long)v + 1;
+        TcMap kvmap;
+        if (attention_tc_make_map(&kvmap, kv, n_pages, Hkv, page_tokens, hd) != 0) {
+            cudaFree(sid); cudaFree(cnt); cudaFree(po); cudaFree(pml);
+            return set_err(SAGC_ECUDA, "cuTensorMapEncodeTiled failed");
+        }
+        r = launch_attention_tc(a, &kvmap, env_int("SAGC_ATT_TC_STAGES", 0), st);
+    } else {
+        r = variant == 1 ? launch_attention_units(a, n_sm, st) : launch_attention(a, st);
+    }
     cudaError_t e = cudaStreamSynchronize(st);
     cudaFree(sid); cudaFree(cnt); cudaFree(po); cudaFree(pml);
     if (r < 0) return set_err(SAGC_EINVAL, "unsupported head_dim %d", hd);

@@ -179,12 +179,14 @@ def _attention_case(rng, ctxs, Hq, Hkv, hd, page):
 
 
 @pytest.mark.parametrize("Hq,Hkv,hd,page", [(4, 4, 32, 16), (14, 2, 64, 64), (28, 4, 128, 64), (8, 1, 128, 32)])
-@pytest.mark.parametrize("splits,variant", [(1, 0), (2, 0), (4, 0), (8, 0), (16, 0), (1, 1), (3, 1), (8, 1), (32, 1)])
+@pytest.mark.parametrize("splits,variant", [(1, 0), (2, 0), (4, 0), (8, 0), (16, 0), (1, 1), (3, 1), (8, 1), (32, 1),
+                                            (1, 2), (2, 2), (5, 2), (12, 2), (64, 2)])
 def test_paged_attention_vs_fp64(B, Hq, Hkv, hd, page, splits, variant):
     """variant 0: the standalone kernel (cluster merge for 2..8 splits, L2 merge for 16); variant 1: the units of the
-    persistent decode-step kernel (its tile geometry, unit loop and last-arriver merge)."""
-    if variant == 1 and hd == 32:
-        pytest.skip("the decode-step kernel serves head_dim 64 / 128")
+    persistent decode-step kernel (its tile geometry, unit loop and last-arriver merge); variant 2: the tcgen05 kernel
+    of the decode steps (TMA-staged pages, S and O in tensor memory, lazy running maximum)."""
+    if variant >= 1 and hd == 32:
+        pytest.skip("the decode-step / tcgen05 kernels serve head_dim 64 / 128")
     rng = np.random.default_rng(Hq * 100 + hd)
     ctxs = np.array([1, 2, page - 1, page, page + 1, 127, 128, 129, 700, 1500], dtype=np.int32)
     q, kv, pt, ref = _attention_case(rng, ctxs, Hq, Hkv, hd, page)
@@ -193,7 +195,8 @@ def test_paged_attention_vs_fp64(B, Hq, Hkv, hd, page, splits, variant):
 
 
 @pytest.mark.parametrize("Hq,Hkv,hd", [(14, 2, 64), (28, 4, 128)])
-@pytest.mark.parametrize("splits,variant", [(1, 0), (2, 0), (4, 0), (8, 0), (16, 0), (1, 1), (8, 1), (18, 1), (32, 1)])
+@pytest.mark.parametrize("splits,variant", [(1, 0), (2, 0), (4, 0), (8, 0), (16, 0), (1, 1), (8, 1), (18, 1), (32, 1),
+                                            (1, 2), (8, 2), (32, 2), (64, 2)])
 def test_paged_attention_long_context(B, Hq, Hkv, hd, splits, variant):
     """The contexts of the full-size configs: 4 095 / 4 352 (cfg2 cap), 8 704 (cfg3/4 cap), 17 408 (cfg5 cap)."""
     rng = np.random.default_rng(hd + splits)
