@@ -21,6 +21,8 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-Xcompiler", "-fPIC"]
 if os.environ.get("SAGC_PDL_EARLY"):
     NVCC_FLAGS += ["-DSAGC_PDL_EARLY"]
+if os.environ.get("SAGC_ATT_TIMELINE"):     # clock64 timeline of the tcgen05 attention kernel (debug builds only)
+    NVCC_FLAGS += ["-DSAGC_ATT_TIMELINE"]
 if os.environ.get("SAGC_TRACE_BUILD"):       # in-kernel timeline (debug builds only)
     NVCC_FLAGS += ["-DSAGC_TRACE", "-rdc=true"]
 

@@ -28,7 +28,7 @@
 
 namespace sagc {
 
-static constexpr int ATC_THREADS = 192;
+static constexpr int ATC_THREADS = 320;       // TMA warp, MMA warp, two softmax warpgroups
 static constexpr int ATC_TILE = 128;
 static constexpr float ATC_LAZY = 8.0f;
 
@@ -40,15 +40,16 @@ struct AttTc {
     static constexpr int MAXSTAGE = HD == 128 ? 3 : 6;              // 192 KB of K/V in flight
     static constexpr int Q_BYTES = HALVES * 16 * 128;               // [half][16 rows][64 bf16]
     static constexpr int P_BYTES = 2 * 16 * 128;                    // [token half][16 rows][64 tokens]
-    static constexpr int tail_bytes() { return Q_BYTES + 2 * P_BYTES; }      // Q and the two P buffers follow the ring
+    static constexpr int tail_bytes() { return Q_BYTES + 4 * P_BYTES; }      // Q and the 2 x 2 P buffers follow the ring
 };
 
 struct AtcSmall {
-    uint64_t kv_full[8], kv_empty[8], s_full[2], p_full[2], p_free[2], q_ready, app_done, o_done;
+    uint64_t kv_full[8], kv_empty[8], s_full[4], p_full[4], p_free[4], q_ready, app_done, o_done;      // [4] = [warpgroup][buffer]
     uint32_t tmem_slot;
     int last_s;
-    float mt_s[2][4][8];            // per-warp tile maxima, double buffered by tile parity
-    float l_s[4][8];
+    float mt_s[4][4][8];            // [2 * warpgroup + buffer][warp][head]: per-warp tile maxima
+    float l_s[2][4][8];
+    float xm[8], xl[8];             // warpgroup 1 -> 0: its running maximum and row sum per head
     float wgt[ATT_MAXR * 64];       // split merge weights [r][nst]
     int pg_s[ATT_MAXPG];
 };
@@ -93,7 +94,67 @@ __device__ __forceinline__ float warp_max_redux(float x) {
     b = b >= 0 ? b : b ^ 0x7fffffff;
     return __int_as_float(b);
 }
-__device__ __forceinline__ void bar_softmax() { asm volatile("bar.sync 1, 128;\n" ::: "memory"); }
+// Warp-converged issue: the TMA and MMA warps run their loops with all 32 lanes (uniform control flow, operands in
+// uniform registers) and one elected lane executes the instruction.  Issuing from inside an `if (lane == 0)` region
+// makes the compiler wrap every UTCHMMA / UTMALDG in an ELECT / R2UR / BRA.U.ANY loop: ~85 cycles per MMA measured.
+__device__ __forceinline__ void tc_mma_e(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accum) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p, pe;\n"
+        "elect.sync _|pe, 0xffffffff;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accum)
+        : "memory");
+}
+__device__ __forceinline__ void tc_commit_e(uint64_t* bar) {
+    asm volatile(
+        "{\n"
+        ".reg .pred pe;\n"
+        "elect.sync _|pe, 0xffffffff;\n"
+        "@pe tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n"
+        "}\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx_e(uint64_t* bar, uint32_t bytes) {
+    asm volatile(
+        "{\n"
+        ".reg .pred pe;\n"
+        "elect.sync _|pe, 0xffffffff;\n"
+        "@pe mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d_e(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1) {
+    asm volatile(
+        "{\n"
+        ".reg .pred pe;\n"
+        "elect.sync _|pe, 0xffffffff;\n"
+        "@pe cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];\n"
+        "}\n" ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+        : "memory");
+}
+
+// non-blocking probe of a phase parity (mbarrier.try_wait may suspend the thread up to a time limit: not for polling two queues)
+__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return ok != 0;
+}
+
+#ifdef SAGC_ATT_TIMELINE
+#define ATC_MARK(role, tile, ev)                                                                                   \
+    do {                                                                                                           \
+        if (a.dbg != nullptr && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && (tile) < 64)              \
+            a.dbg[((role) * 64 + (tile)) * 8 + (ev)] = clock64();                                                  \
+    } while (0)
+#else
+#define ATC_MARK(role, tile, ev) ((void)0)
+#endif
+__device__ __forceinline__ void bar_softmax(int wg) { asm volatile("bar.sync %0, 128;\n" ::"r"(1 + wg) : "memory"); }
 
 template <int HD>
 __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_constant__ CUtensorMap kvmap, AttnArgs a, int NS) {
@@ -102,7 +163,7 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
     unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     unsigned char* q_s = smem + (size_t)NS * C::KV_BYTES;
     unsigned char* p_s = q_s + C::Q_BYTES;
-    AtcSmall* sm = reinterpret_cast<AtcSmall*>(p_s + 2 * C::P_BYTES);
+    AtcSmall* sm = reinterpret_cast<AtcSmall*>(p_s + 4 * C::P_BYTES);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     // decode (a.prefetch): the live list, contexts, page table and every cached position but the newest predate the
     // upstream kernel (this step's QKV projection); only q and the new k, v must wait for it
@@ -129,13 +190,13 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
 
     if (tid == 0) {
         for (int s = 0; s < NS; ++s) { mbar_init(&sm->kv_full[s], 1); mbar_init(&sm->kv_empty[s], 1); }
-        for (int b = 0; b < 2; ++b) { mbar_init(&sm->s_full[b], 1); mbar_init(&sm->p_full[b], 4); mbar_init(&sm->p_free[b], 1); }
+        for (int b = 0; b < 4; ++b) { mbar_init(&sm->s_full[b], 1); mbar_init(&sm->p_full[b], 4); mbar_init(&sm->p_free[b], 1); }
         mbar_init(&sm->q_ready, 4); mbar_init(&sm->app_done, 4); mbar_init(&sm->o_done, 1);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
         tma_prefetch_desc(&kvmap);
     }
     if (warp == 1) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&sm->tmem_slot)), "n"(64));
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&sm->tmem_slot)), "n"(128));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n");
     }
     if (pg_cached)
@@ -144,85 +205,115 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = sm->tmem_slot;
-    const uint32_t tm_s[2] = {tmem_base, tmem_base + 16};
-    const uint32_t tm_o = tmem_base + 32;
+    if (tid == 0) ATC_MARK(0, 63, 0);
+    // tensor memory columns: S^T of (warpgroup g, buffer b) at 16 * (2g + b); O^T of warpgroup g at 64 + 16 g
+    // tile i belongs to warpgroup i & 1; it is that warpgroup's tile j = i >> 1 and uses its buffer j & 1
 
     if (warp == 0) {
         // ===== TMA producer =====================================================================
-        if (lane == 0 && n_tiles > 0) {
+        if (n_tiles > 0) {                                       // all 32 lanes, converged
             const int ppt = ATC_TILE >> pshift;                  // pages per tile
             const uint32_t box_bytes = (uint32_t)a.page * 128u;
             for (int i = 0; i < n_tiles; ++i) {
                 const int s = i % NS, k = i / NS;
                 mbar_wait(&sm->kv_empty[s], (uint32_t)((k & 1) ^ 1));
                 if (designated && i == n_tiles - 1) mbar_wait(&sm->app_done, 0);      // the new K,V row is in the pool
-                mbar_expect_tx(&sm->kv_full[s], (uint32_t)C::KV_BYTES);
+                if (lane == 0) ATC_MARK(0, i, 0);
+                mbar_expect_tx_e(&sm->kv_full[s], (uint32_t)C::KV_BYTES);
                 unsigned char* st = smem + (size_t)s * C::KV_BYTES;
                 const int blk0 = (t_begin + i * ATC_TILE) >> pshift;
-                for (int p = 0; p < ppt; ++p) {
-                    const int blk = min(blk0 + p, last_blk);          // past the context: any finite page (masked, p = 0)
-                    int pg = pg_cached ? sm->pg_s[blk - b_begin] : pt[blk];
-                    if (pg < 0) pg = 0;                               // unmapped block after a pool-exhaustion error
-                    const int row_k = ((pg * 2 + 0) * a.Hkv + kvh) * a.page;
-                    const int row_v = ((pg * 2 + 1) * a.Hkv + kvh) * a.page;
+                for (int p0 = 0; p0 < ppt; p0 += 2) {            // two pages at a time: their page ids and rows first, then the copies
+                    int row_v[2];
 #pragma unroll
-                    for (int h = 0; h < C::HALVES; ++h) {
-                        tma_load_2d(st + (size_t)h * C::HALF_BYTES + (size_t)p * box_bytes, &kvmap, &sm->kv_full[s], h * 64, row_v);
-                        tma_load_2d(st + (size_t)(C::HALVES + h) * C::HALF_BYTES + (size_t)p * box_bytes, &kvmap, &sm->kv_full[s], h * 64, row_k);
+                    for (int u = 0; u < 2; ++u) {
+                        const int blk = min(blk0 + p0 + u, last_blk);      // past the context: any finite page (masked, p = 0)
+                        int pg = pg_cached ? sm->pg_s[blk - b_begin] : pt[blk];
+                        if (pg < 0) pg = 0;                                // unmapped block after a pool-exhaustion error
+                        row_v[u] = ((pg * 2 + 1) * a.Hkv + kvh) * a.page;
+                    }
+                    const int k_off = a.Hkv * a.page;                      // the K slab sits Hkv slabs before the V slab
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        if (p0 + u >= ppt) break;
+                        unsigned char* dst = st + (size_t)(p0 + u) * box_bytes;
+#pragma unroll
+                        for (int h = 0; h < C::HALVES; ++h) {
+                            tma_load_2d_e(dst + (size_t)h * C::HALF_BYTES, &kvmap, &sm->kv_full[s], h * 64, row_v[u]);
+                            tma_load_2d_e(dst + (size_t)(C::HALVES + h) * C::HALF_BYTES, &kvmap, &sm->kv_full[s], h * 64, row_v[u] - k_off);
+                        }
                     }
                 }
+                if (lane == 0) ATC_MARK(0, i, 1);
             }
         }
     } else if (warp == 1) {
         // ===== MMA issuer =======================================================================
-        if (lane == 0 && n_tiles > 0) {
+        if (n_tiles > 0) {                                       // all 32 lanes, converged
             const uint32_t idesc_s = umma_idesc(16);                        // S^T: M = 128 tokens, N = 16, A and B K-major
             const uint32_t idesc_o = umma_idesc(16) | (1u << 15);           // O^T: M = 128 (d), N = 16, A MN-major
             const uint32_t q_a = smem_u32(q_s), p_a = smem_u32(p_s);
-            auto issue_pv = [&](int j) {
-                const int b = j & 1, s = j % NS;
-                mbar_wait(&sm->p_full[b], (uint32_t)((j >> 1) & 1));
-                tc_fence_after();
-                const uint32_t v_a = smem_u32(smem + (size_t)s * C::KV_BYTES);
-#pragma unroll
-                for (int ks = 0; ks < ATC_TILE / 16; ++ks) {
-                    const uint64_t da = umma_desc_mn_sw128(v_a + ks * 2048, C::HALF_BYTES);
-                    const uint64_t db = umma_desc_sw128(p_a + b * C::P_BYTES + (ks >> 2) * 2048 + (ks & 3) * 32);
-                    tc_mma(tm_o, da, db, idesc_o, (j > 0 || ks > 0) ? 1u : 0u);
-                }
-                tc_commit(&sm->kv_empty[s]);
-                tc_commit(&sm->p_free[b]);
-            };
             mbar_wait(&sm->q_ready, 0);
             tc_fence_after();
-            for (int i = 0; i < n_tiles; ++i) {
-                const int s = i % NS;
-                mbar_wait(&sm->kv_full[s], (uint32_t)((i / NS) & 1));
-                tc_fence_after();
-                const uint32_t k_a = smem_u32(smem + (size_t)s * C::KV_BYTES + (size_t)C::HALVES * C::HALF_BYTES);
+            // Two independent queues served by whichever is ready (a blocking wait on one would hold the other up and,
+            // through the K/V ring, starve itself): S of tile is (needs its K/V tile and a free S buffer: S of tile
+            // is - 4 has been consumed once p_full of that tile was seen), P.V of tile ip (needs that tile's P).
+            int is = 0, ip = 0;
+            while (ip < n_tiles) {
+                bool idle = true;
+                if (is < n_tiles && is < ip + 4) {
+                    const int s = is % NS;
+                    if (__any_sync(0xffffffffu, mbar_test(&sm->kv_full[s], (uint32_t)((is / NS) & 1)))) {
+                        if (lane == 0) ATC_MARK(1, is, 1);
+                        tc_fence_after();
+                        const uint32_t k_a = smem_u32(smem + (size_t)s * C::KV_BYTES + (size_t)C::HALVES * C::HALF_BYTES);
+                        const int sb = 2 * (is & 1) + ((is >> 1) & 1);
 #pragma unroll
-                for (int ks = 0; ks < HD / 16; ++ks) {
-                    const uint64_t da = umma_desc_sw128(k_a + (ks >> 2) * C::HALF_BYTES + (ks & 3) * 32);
-                    const uint64_t db = umma_desc_sw128(q_a + (ks >> 2) * 2048 + (ks & 3) * 32);
-                    tc_mma(tm_s[i & 1], da, db, idesc_s, ks > 0 ? 1u : 0u);
+                        for (int ks = 0; ks < HD / 16; ++ks) {
+                            const uint64_t da = umma_desc_sw128(k_a + (ks >> 2) * C::HALF_BYTES + (ks & 3) * 32);
+                            const uint64_t db = umma_desc_sw128(q_a + (ks >> 2) * 2048 + (ks & 3) * 32);
+                            tc_mma_e(tmem_base + 16 * sb, da, db, idesc_s, ks > 0 ? 1u : 0u);
+                        }
+                        tc_commit_e(&sm->s_full[sb]);
+                        if (lane == 0) ATC_MARK(1, is, 2);
+                        ++is;
+                        idle = false;
+                    }
                 }
-                tc_commit(&sm->s_full[i & 1]);
-                if (i > 0) issue_pv(i - 1);
+                if (ip < is) {
+                    const int g = ip & 1, j = ip >> 1, pb = 2 * g + (j & 1), s = ip % NS;
+                    if (__any_sync(0xffffffffu, mbar_test(&sm->p_full[pb], (uint32_t)((j >> 1) & 1)))) {
+                        if (lane == 0) ATC_MARK(1, ip, 3);
+                        tc_fence_after();
+                        const uint32_t v_a = smem_u32(smem + (size_t)s * C::KV_BYTES);
+#pragma unroll
+                        for (int ks = 0; ks < ATC_TILE / 16; ++ks) {
+                            const uint64_t da = umma_desc_mn_sw128(v_a + ks * 2048, C::HALF_BYTES);
+                            const uint64_t db = umma_desc_sw128(p_a + pb * C::P_BYTES + (ks >> 2) * 2048 + (ks & 3) * 32);
+                            tc_mma_e(tmem_base + 64 + 16 * g, da, db, idesc_o, (j > 0 || ks > 0) ? 1u : 0u);
+                        }
+                        tc_commit_e(&sm->kv_empty[s]);
+                        tc_commit_e(&sm->p_free[pb]);
+                        if (lane == 0) ATC_MARK(1, ip, 4);
+                        ++ip;
+                        idle = false;
+                    }
+                }
+                if (idle) __nanosleep(32);         // leave the issue slots of this scheduler to the softmax warps
             }
-            issue_pv(n_tiles - 1);
-            tc_commit(&sm->o_done);
+            tc_commit_e(&sm->o_done);
         }
     } else {
         // ===== softmax warps: thread = token lane of S^T, = output column d of O^T ================
-        const int st = tid - 64;                          // 0..127
-        const int sw = warp - 2;                          // slot in the per-warp scratch
+        const int wg = (warp - 2) >> 2;                   // warpgroup 0 takes the even tiles, 1 the odd ones
+        const int st = (tid - 64) & 127;                  // 0..127 inside the warpgroup
+        const int sw = (warp - 2) & 3;                    // slot in the per-warp scratch
         const int quad = warp & 3;                        // TMEM lane quadrant this warp may access
         const int tl = quad * 32 + lane;                  // token inside the tile / d inside the head
         const uint32_t lane_off = (uint32_t)(quad * 32) << 16;
         // ---- q: RoPE, 1/sqrt(hd), hi / lo split into the swizzled B operand; append of the new k, v ----
         if (a.prefetch) pdl_wait();
         pdl_launch();
-        {
+        if (wg == 0) {
             constexpr int CH = HD / 8;                    // 16-byte chunks per head row
             const int h = st / CH, c = st % CH;
             if (h < 8) {
@@ -284,12 +375,15 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
         float m_used[8], l_part[8];
 #pragma unroll
         for (int h = 0; h < 8; ++h) { m_used[h] = -INFINITY; l_part[h] = 0.f; }
-        for (int i = 0; i < n_tiles; ++i) {
-            const int b = i & 1, k = i >> 1;
+        const uint32_t tm_o = tmem_base + 64 + 16 * wg;
+        for (int i = wg; i < n_tiles; i += 2) {
+            const int j = i >> 1, b = 2 * wg + (j & 1), k = j >> 1;
+            if (st == 0) ATC_MARK(2 + wg, i, 0);
             mbar_wait(&sm->s_full[b], (uint32_t)(k & 1));
+            if (st == 0) ATC_MARK(2 + wg, i, 1);
             tc_fence_after();
             float sv[16];
-            tc_ld16(tm_s[b] + lane_off, sv);
+            tc_ld16(tmem_base + 16 * b + lane_off, sv);
             float s[8];
             const bool valid = t_begin + i * ATC_TILE + tl < t_end;
 #pragma unroll
@@ -303,7 +397,9 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
                     *reinterpret_cast<float4*>(&sm->mt_s[b][sw][4]) = make_float4(wm[4], wm[5], wm[6], wm[7]);
                 }
             }
-            bar_softmax();
+            if (st == 0) ATC_MARK(2 + wg, i, 2);
+            bar_softmax(wg);
+            if (st == 0) ATC_MARK(2 + wg, i, 3);
             float mt[8];
             bool need = false;
 #pragma unroll
@@ -320,8 +416,8 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
                     m_used[h] = mn;
                     l_part[h] *= f[h];
                 }
-                if (i > 0) {                                  // O holds tiles 0 .. i-1 once P.V of tile i-1 has completed
-                    mbar_wait(&sm->p_free[(i - 1) & 1], (uint32_t)(((i - 1) >> 1) & 1));
+                if (j > 0) {                                  // O holds this warpgroup's earlier tiles once P.V of its tile j-1 has completed
+                    mbar_wait(&sm->p_free[2 * wg + ((j - 1) & 1)], (uint32_t)(((j - 1) >> 1) & 1));
                     tc_fence_after();
                     float ov[16];
                     tc_ld16(tm_o + lane_off, ov);
@@ -338,7 +434,9 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
                 ph[h] = f32_to_bf16_bits(p);
                 pl[h] = f32_to_bf16_bits(p - __uint_as_float(ph[h] << 16));
             }
-            mbar_wait(&sm->p_free[b], (uint32_t)((k & 1) ^ 1));      // P.V of tile i-2 has read this buffer
+            if (st == 0) ATC_MARK(2 + wg, i, 4);
+            mbar_wait(&sm->p_free[b], (uint32_t)((k & 1) ^ 1));      // P.V of this warpgroup's tile j-2 has read this buffer
+            if (st == 0) ATC_MARK(2 + wg, i, 5);
             {
                 unsigned char* pb = p_s + b * C::P_BYTES + (tl >> 6) * 2048 + (tl & 7) * 2;
                 const int ch = (tl & 63) >> 3;
@@ -352,12 +450,16 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(&sm->p_full[b]);
+            if (st == 0) ATC_MARK(2 + wg, i, 6);
         }
         // ---- epilogue: O^T columns h (hi) + 8+h (lo) of this thread's d; row sums over the 128 token lanes ----
         float ov[8], l[8];
+        if (st == 0) ATC_MARK(2 + wg, 62, 0);
         if (n_tiles > 0) {
-            mbar_wait(&sm->o_done, 0);
+            mbar_wait(&sm->o_done, 0);            // every P.V has completed: both O accumulators are final, the P buffers free
             tc_fence_after();
+        }
+        if (n_tiles > wg) {
             float o16[16];
             tc_ld16(tm_o + lane_off, o16);
 #pragma unroll
@@ -369,12 +471,35 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
 #pragma unroll
         for (int h = 0; h < 8; ++h) l[h] = warp_sum(l_part[h]);
         if (lane == 0) {
-            *reinterpret_cast<float4*>(&sm->l_s[sw][0]) = make_float4(l[0], l[1], l[2], l[3]);
-            *reinterpret_cast<float4*>(&sm->l_s[sw][4]) = make_float4(l[4], l[5], l[6], l[7]);
+            *reinterpret_cast<float4*>(&sm->l_s[wg][sw][0]) = make_float4(l[0], l[1], l[2], l[3]);
+            *reinterpret_cast<float4*>(&sm->l_s[wg][sw][4]) = make_float4(l[4], l[5], l[6], l[7]);
         }
-        bar_softmax();
+        bar_softmax(wg);
 #pragma unroll
-        for (int h = 0; h < 8; ++h) l[h] = (sm->l_s[0][h] + sm->l_s[1][h]) + (sm->l_s[2][h] + sm->l_s[3][h]);
+        for (int h = 0; h < 8; ++h) l[h] = (sm->l_s[wg][0][h] + sm->l_s[wg][1][h]) + (sm->l_s[wg][2][h] + sm->l_s[wg][3][h]);
+        // ---- the odd tiles' (o, m, l) join the even tiles' (same log-sum-exp rule as the split merge) ----
+        float* xo = reinterpret_cast<float*>(p_s);          // [d][8], overlays the P buffers
+        if (wg == 1) {
+#pragma unroll
+            for (int h = 0; h < 8; h += 4) *reinterpret_cast<float4*>(xo + tl * 8 + h) = make_float4(ov[h], ov[h + 1], ov[h + 2], ov[h + 3]);
+            if (st == 0) {
+#pragma unroll
+                for (int h = 0; h < 8; ++h) { sm->xm[h] = m_used[h]; sm->xl[h] = l[h]; }
+            }
+        }
+        if (st == 0) ATC_MARK(2 + wg, 62, 1);
+        asm volatile("bar.sync 3, 256;\n" ::: "memory");
+        if (st == 0) ATC_MARK(2 + wg, 62, 2);
+        if (wg == 0) {
+#pragma unroll
+        for (int h = 0; h < 8; ++h) {
+            const float mb = sm->xm[h], mn = fmaxf(m_used[h], mb);
+            const float fa = (m_used[h] == -INFINITY) ? 0.f : __expf(m_used[h] - mn);
+            const float fb = (mb == -INFINITY) ? 0.f : __expf(mb - mn);
+            ov[h] = ov[h] * fa + xo[tl * 8 + h] * fb;
+            l[h] = l[h] * fa + sm->xl[h] * fb;
+            m_used[h] = mn;
+        }
         if (nsp == 1) {
             if (tl < HD) {
 #pragma unroll
@@ -394,13 +519,16 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
                     ml[0] = m_used[h];
                     ml[1] = l[h];
                 }
+            if (st == 0) ATC_MARK(2, 62, 3);
             __threadfence();
-            bar_softmax();
+            bar_softmax(0);
+            if (st == 0) ATC_MARK(2, 62, 4);
             if (st == 0) {
                 const int prev = atomicAdd(&a.counters[row * a.Hkv + kvh], 1);
                 sm->last_s = (prev == nsp - 1);
             }
-            bar_softmax();
+            bar_softmax(0);
+            if (st == 0) ATC_MARK(2, 62, 5);
             if (sm->last_s) {
                 // ---- merge: this unit arrived last for (row, kv head); arithmetic of attention_body.cuh ----
                 __threadfence();
@@ -422,24 +550,44 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
                     for (int u = 0; u < 2; ++u)
                         if (lane + 32 * u < nsp) sm->wgt[h * nsp + lane + 32 * u] = f[u] / den;
                 }
-                bar_softmax();
-                if (tl < HD) {
-                    for (int h = 0; h < r; ++h) {
-                        const int hq = kvh * r + h;
-                        const float* po = a.part_o + ((size_t)row * a.Hq + hq) * nsp * HD + tl;
-                        float num = 0.f;
-#pragma unroll 4
-                        for (int s2 = 0; s2 < nsp; ++s2) num += sm->wgt[h * nsp + s2] * __ldcg(po + (size_t)s2 * HD);
-                        store_out(a, row, hq * HD + tl, num);
+                bar_softmax(0);
+                // every thread combines r * HD / 128 outputs; the loads of 8 splits x 2 outputs are in flight together
+                // (the partials sit in L2: the merge is a chain of round trips, not bandwidth)
+                const int n_out = r * HD;
+                for (int i0 = st; i0 < n_out; i0 += 256) {
+                    const int i1 = i0 + 128;
+                    const bool two = i1 < n_out;
+                    const int h0 = i0 / HD, d0 = i0 % HD, h1 = two ? i1 / HD : h0, d1 = two ? i1 % HD : d0;
+                    const float* po0 = a.part_o + ((size_t)row * a.Hq + kvh * r + h0) * nsp * HD + d0;
+                    const float* po1 = a.part_o + ((size_t)row * a.Hq + kvh * r + h1) * nsp * HD + d1;
+                    const float* w0 = sm->wgt + h0 * nsp;
+                    const float* w1 = sm->wgt + h1 * nsp;
+                    float n0 = 0.f, n1 = 0.f;
+                    for (int s0 = 0; s0 < nsp; s0 += 8) {
+                        float v0[8], v1[8];
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) {
+                            const int s2 = min(s0 + u, nsp - 1);
+                            v0[u] = __ldcg(po0 + (size_t)s2 * HD);
+                            v1[u] = __ldcg(po1 + (size_t)s2 * HD);
+                        }
+#pragma unroll
+                        for (int u = 0; u < 8; ++u)
+                            if (s0 + u < nsp) { n0 += w0[s0 + u] * v0[u]; n1 += w1[s0 + u] * v1[u]; }
                     }
+                    store_out(a, row, (kvh * r + h0) * HD + d0, n0);
+                    if (two) store_out(a, row, (kvh * r + h1) * HD + d1, n1);
                 }
+                if (st == 0) ATC_MARK(2, 62, 6);
                 if (st == 0) a.counters[row * a.Hkv + kvh] = 0;
             }
         }
+        }   // warpgroup 0
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "n"(64));
+    if (tid == 0) ATC_MARK(0, 63, 1);
+    if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "n"(128));
 }
 
 template <int HD>

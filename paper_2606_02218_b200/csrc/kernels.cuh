@@ -77,6 +77,7 @@ struct AttnArgs {
     const long long* q_fx; const float* q_rstd;
     int prefetch;           // 1 in decode: cached positions older than the newest one predate the upstream kernel
     int cluster_merge;      // set by the launcher: the n_splits CTAs of a (row, kv head) form a cluster and merge through DSMEM
+    unsigned long long* dbg; // attention_tc.cu built with -DSAGC_ATT_TIMELINE: clock64 stamps of CTA (0,0,0), [role 4][tile 64][event 8]; else unused
 };
 int launch_attention(const AttnArgs& a, cudaStream_t st);
 

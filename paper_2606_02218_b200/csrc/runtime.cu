@@ -215,7 +215,9 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
         sagc_model_destroy(m);
         return set_err(SAGC_ECUDA, "cudaMemset of the KV pool failed");
     }
-    m->att_tc = env_int("SAGC_ATT_TC", 1) && attention_tc_supports(c.head_dim, c.page_tokens, c.n_q_heads / c.n_kv_heads);
+    // measured (profiles/r02_attention.md): the tcgen05 kernel wins at head_dim 128 (7B shape: 1.3 - 1.6x in the tail, 1.35x at 256
+    // rows); at head_dim 64 its per-tile gain does not pay for its longer prologue / epilogue at the short contexts of those models
+    m->att_tc = env_int("SAGC_ATT_TC", c.head_dim == 128 ? 1 : 0) && attention_tc_supports(c.head_dim, c.page_tokens, c.n_q_heads / c.n_kv_heads);
     m->att_tc_stages = env_int("SAGC_ATT_TC_STAGES", 0);
     if (m->att_tc) {
         m->kvmaps.resize(L > 0 ? L : 1);
@@ -545,11 +547,12 @@ static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
     if (s > smax) s = smax;
     if (m->att_tc && m->cfg.head_dim >= 64) {
         // tcgen05 decode attention: one CTA per SM (the K/V ring fills shared memory), >= 2 tiles of 128 tokens per
-        // split, partials merged through L2 by the last arriver (no cluster limit)
+        // split, partials merged through L2 by the last arriver; more than 16 splits cost more in the merge than they
+        // save in the scan (1 row x 16 000 tokens: 26 us with 16 splits, 30 us with 32)
         int w2 = sagc::g_num_sms / ctas;
         const int cap2 = ctx_bound / 256;
         if (w2 > cap2) w2 = cap2;
-        if (w2 > 32) w2 = 32;
+        if (w2 > 16) w2 = 16;
         if (w2 > m->max_splits) w2 = m->max_splits;
         s = 1;
         while (s * 2 <= w2) s *= 2;
@@ -1278,7 +1281,30 @@ extern "C" int sagc_debug_attention(const float* q, const void* kv, const int32_
             cudaFree(sid); cudaFree(cnt); cudaFree(po); cudaFree(pml);
             return set_err(SAGC_ECUDA, "cuTensorMapEncodeTiled failed");
         }
+        unsigned long long* dbg = nullptr;
+        if (env_int("SAGC_ATT_DBG", 0)) {        // timeline of CTA (0,0,0): needs a library built with SAGC_ATT_TIMELINE=1
+            CU(cudaMalloc(&dbg, 4 * 64 * 8 * sizeof(unsigned long long)));
+            CU(cudaMemsetAsync(dbg, 0, 4 * 64 * 8 * sizeof(unsigned long long), st));
+            a.dbg = dbg;
+        }
         r = launch_attention_tc(a, &kvmap, env_int("SAGC_ATT_TC_STAGES", 0), st);
+        if (dbg) {
+            std::vector<unsigned long long> h(4 * 64 * 8);
+            cudaStreamSynchronize(st);
+            cudaMemcpy(h.data(), dbg, h.size() * 8, cudaMemcpyDeviceToHost);
+            cudaFree(dbg);
+            unsigned long long t0 = ~0ull;
+            for (auto v : h) if (v && v < t0) t0 = v;
+            for (int role = 0; role < 4; ++role)
+                for (int tile = 0; tile < 64; ++tile) {
+                    bool any = false;
+                    for (int e = 0; e < 8; ++e) any |= h[(role * 64 + tile) * 8 + e] != 0;
+                    if (!any) continue;
+                    fprintf(stderr, "ATC role %d tile %2d:", role, tile);
+                    for (int e = 0; e < 8; ++e) { auto v = h[(role * 64 + tile) * 8 + e]; fprintf(stderr, " %7lld", v ? (long long)(v - t0) : -1LL); }
+                    fprintf(stderr, "\n");
+                }
+        }
     } else {
         r = variant == 1 ? launch_attention_units(a, n_sm, st) : launch_attention(a, st);
     }
