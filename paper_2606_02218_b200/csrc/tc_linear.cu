@@ -40,6 +40,7 @@ struct TcDev {
     const float* ssq_in; int ssq_in_tiles;   // fused RMSNorm of the INPUT: rstd[m] from these partials
     int ssq_ld; float eps; int k_norm;
     int stages;                     // smem ring depth chosen by the launcher
+    int mtiles;                     // batch tiles of MB rows; blockIdx.x = weight tile * mtiles + batch tile
     float* scratch;                 // split-K partial tiles [cta][NA][MB][128] (L2-resident), KS > 1 only
     // EPI_QKV (fused RoPE + KV append)
     const float* rope_cs; const int* row_pos; const int* row_sid; const int* page_table; bf16_t* kv_layer;
@@ -274,9 +275,12 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     const int rank = (int)cluster.block_rank();
     const int KS = (int)cluster.num_blocks();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int tile = blockIdx.x, row0 = tile * 128;
-    const int m0 = blockIdx.z * MB;
-    const int cta_id = ((int)blockIdx.z * (int)gridDim.x + (int)blockIdx.x) * KS + rank;
+    // the batch tiles of one weight tile are NEIGHBOURS in launch order: they run in the same wave, so the weight tile
+    // comes from DRAM once and the other batch tiles hit L2 (with batch tiles in grid.z every wave re-read the matrix:
+    // dram__bytes_read was 2x the weights at 256 rows, profiles/r02_ncu_top_kernels.md)
+    const int tile = (int)blockIdx.x / a.mtiles, row0 = tile * 128;
+    const int m0 = ((int)blockIdx.x % a.mtiles) * MB;
+    const int cta_id = (int)blockIdx.x * KS + rank;
     const int kb0 = rank * a.kb_per_cta;
     const int nk = max(0, min(a.n_kb, kb0 + a.kb_per_cta) - kb0);
 
@@ -547,7 +551,8 @@ int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
     if (t.scratch == nullptr) KS = 1;
     { int p2 = 1; while (p2 * 2 <= KS) p2 *= 2; KS = p2; }      // the epilogue is specialised for 1, 2, 4, 8
     d.kb_per_cta = (d.n_kb + KS - 1) / KS;             // trailing ranks may get fewer (or zero) k blocks
-    dim3 grid(tiles, KS, mtiles);
+    d.mtiles = mtiles;
+    dim3 grid(tiles * mtiles, KS, 1);
     cudaError_t e;
 #define TC_CASE(NBV)                                                                         \
     case NBV:                                                                                \
