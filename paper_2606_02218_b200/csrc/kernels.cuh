@@ -53,6 +53,13 @@ struct RopeArgs {
 int launch_rope_append(const RopeArgs& a, cudaStream_t st);
 
 // Paged GQA attention over ragged contexts with split-K + in-kernel LSE merge.  Step a7.
+struct TcPf {
+    const void* maps;       // device CUtensorMap[n_maps], consecutive, box 64 x 128 (null = off)
+    int n_maps;
+    int tiles[3];           // 128-row tiles of each map
+    int ks, kbpc, nkb;      // next kernel: K-split ranks, 64-wide k blocks per rank, leading blocks to fetch per (tile, rank)
+};
+
 struct AttnArgs {
     const float* q;         // [M][ldq] (first Hq*hd columns are the rotated queries)
     int ldq;
@@ -77,6 +84,7 @@ struct AttnArgs {
     const long long* q_fx; const float* q_rstd;
     int prefetch;           // 1 in decode: cached positions older than the newest one predate the upstream kernel
     int cluster_merge;      // set by the launcher: the n_splits CTAs of a (row, kv head) form a cluster and merge through DSMEM
+    TcPf pf;                // attention_tc.cu: L2 prefetch of the next GEMM's leading weight blocks (maps == null: off)
     unsigned long long* dbg; // attention_tc.cu built with -DSAGC_ATT_TIMELINE: clock64 stamps of CTA (0,0,0), [role 4][tile 64][event 8]; else unused
 };
 int launch_attention(const AttnArgs& a, cudaStream_t st);
@@ -155,6 +163,8 @@ int launch_dump_logits(const int* dump_sid_t, int n_dump, const int* step_dev, c
 struct alignas(64) TcMap { unsigned char opaque[128]; };     // mirrors CUtensorMap
 int tc_make_map(TcMap* out, const void* base, long long rows, int K, int box_rows);
 int tc_nb_index(int m_max);                                  // 0..3 -> UMMA N = 32, 64, 128, 256
+// K-split ranks and k blocks per rank that launch_linear_tc will use for a GEMM of this shape (so that the PREVIOUS kernel can prefetch its streams)
+int tc_plan(int N, int K, int m_max, bool swiglu, bool has_scratch, int* kb_per_cta);
 static constexpr size_t TC_SCRATCH_FLOATS = (size_t)296 * 2 * 128 * 128;   // 296 CTAs x NA 2 x 128 cols x 128 rows
 struct TcLinearArgs {
     const TcMap* a[3];          // weight maps (box 64 x 128): {w} | {q, k, v} | {gate, up}
@@ -163,6 +173,7 @@ struct TcLinearArgs {
     int K, N;                   // N = output rows (EPI_SWIGLU: d_ff)
     const int* m_dev; int m_max;
     int epi;
+    TcPf pf;                    // L2 prefetch of the NEXT GEMM's leading weight blocks, issued after this kernel's own loads (maps == null: off)
     float* Y; int ldy; const float* R;
     bf16_t* xs_out; int ld_xs; const bf16_t* norm_next; float* ssq_out;
     const float* ssq_in; int ssq_in_tiles; int ssq_ld; float eps; int k_norm;

@@ -40,6 +40,7 @@ struct TcDev {
     const float* ssq_in; int ssq_in_tiles;   // fused RMSNorm of the INPUT: rstd[m] from these partials
     int ssq_ld; float eps; int k_norm;
     int stages;                     // smem ring depth chosen by the launcher
+    TcPf pf;                        // next GEMM's weight streams to prefetch into L2
     int mtiles;                     // batch tiles of MB rows; blockIdx.x = weight tile * mtiles + batch tile
     float* scratch;                 // split-K partial tiles [cta][NA][MB][128] (L2-resident), KS > 1 only
     // EPI_QKV (fused RoPE + KV append)
@@ -361,6 +362,9 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             }
             __syncwarp();
         }
+        // every MMA of this CTA is issued, so its weight stream has landed: from here to the next kernel's first loads the
+        // bus would idle (epilogue, cluster reduction, the next prologue) -- fetch the next GEMM's leading blocks into L2
+        if (lane == 0) tc_prefetch_next(a.pf, cta_id, (int)gridDim.x * KS);
     } else {
         // ===== epilogue warps: TMEM -> (hi + lo) -> shared reduce buffer =====
         const int lg = warp & 3;                      // TMEM lane group of this warp
@@ -524,9 +528,31 @@ static cudaError_t launch_tc_inst(const TcLinearArgs& t, const TcDev& d, dim3 gr
 
 int tc_nb_index(int m_max) { return m_max <= 16 ? 0 : (m_max <= 32 ? 1 : (m_max <= 64 ? 2 : 3)); }
 
+int tc_plan(int N, int K, int m_max, bool swiglu, bool has_scratch, int* kb_per_cta) {
+    const int nbi = tc_nb_index(m_max);
+    const int MB = (32 << nbi) / 2;
+    const int tiles = N / 128, mtiles = (m_max + MB - 1) / MB, n_kb = K / TC_BK;
+    // K-split policy (measured with the in-kernel timeline): a CTA streams its weight slab through a deep
+    // TMA ring at well over 150 GB/s, while every extra cluster rank adds DSMEM round trips to the
+    // epilogue -- so K is split down to ~30 KB slabs per CTA (swept on cfg2), in powers of two up to 8, and never beyond two CTAs per SM.
+    const double slab = (swiglu ? 2.0 : 1.0) * 128.0 * K * 2.0;
+    const double slab_max = 30.0e3;
+    int KS = (int)((slab + slab_max - 1) / slab_max);
+    const int room = (2 * g_num_sms) / (tiles * mtiles);
+    if (KS > room) KS = room;
+    if (KS < 1) KS = 1;
+    if (KS > 8) KS = 8;     // cap re-swept in round 2 (decode step, cap 8 / 4 / 2): 1.5B 1.42 / - / 1.80 ms, 7B 3.35 / 3.60 / 5.06 ms
+    if (KS > n_kb) KS = n_kb;
+    if (!has_scratch) KS = 1;
+    { int p2 = 1; while (p2 * 2 <= KS) p2 *= 2; KS = p2; }      // the epilogue is specialised for 1, 2, 4, 8
+    if (kb_per_cta) *kb_per_cta = (n_kb + KS - 1) / KS;            // trailing ranks may get fewer (or zero) k blocks
+    return KS;
+}
+
 int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
     if (t.m_max <= 0) return 0;
     TcDev d;
+    d.pf = t.pf;
     d.K = t.K; d.N = t.N; d.n_kb = t.K / TC_BK; d.m_dev = t.m_dev; d.m_max = t.m_max; d.Y = t.Y; d.ldy = t.ldy; d.R = t.R;
     d.xs_out = t.xs_out; d.ld_xs = t.ld_xs; d.norm_next = t.norm_next; d.ssq_out = t.ssq_out; d.ssq_in = t.ssq_in;
     d.ssq_in_tiles = t.ssq_in_tiles; d.ssq_ld = t.ssq_ld; d.eps = t.eps; d.k_norm = t.k_norm; d.scratch = t.scratch;
@@ -535,22 +561,8 @@ int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
     const int nbi = tc_nb_index(t.m_max);
     const int NB = 32 << nbi, MB = NB / 2;
     const int tiles = t.N / 128, mtiles = (t.m_max + MB - 1) / MB;
-    // K-split policy (measured with the in-kernel timeline): a CTA streams its weight slab through a deep
-    // TMA ring at well over 150 GB/s, while every extra cluster rank adds DSMEM round trips to the
-    // epilogue -- so K is split down to ~30 KB slabs per CTA (swept on cfg2), in powers of two up to 8, and never beyond two CTAs per SM.
-    const int NAh = (t.epi == EPI_SWIGLU) ? 2 : 1;
-    const double slab = (double)NAh * 128.0 * t.K * 2.0;
-    const double slab_max = 30.0e3;
-    int KS = (int)((slab + slab_max - 1) / slab_max);
-    const int room = (2 * g_num_sms) / (tiles * mtiles);
     if ((size_t)2 * g_num_sms * 2 * 128 * 128 > TC_SCRATCH_FLOATS) return -1;      // split-K scratch is sized for 296 CTAs
-    if (KS > room) KS = room;
-    if (KS < 1) KS = 1;
-    if (KS > 8) KS = 8;     // cap re-swept in round 2 (decode step, cap 8 / 4 / 2): 1.5B 1.42 / - / 1.80 ms, 7B 3.35 / 3.60 / 5.06 ms
-    if (KS > d.n_kb) KS = d.n_kb;
-    if (t.scratch == nullptr) KS = 1;
-    { int p2 = 1; while (p2 * 2 <= KS) p2 *= 2; KS = p2; }      // the epilogue is specialised for 1, 2, 4, 8
-    d.kb_per_cta = (d.n_kb + KS - 1) / KS;             // trailing ranks may get fewer (or zero) k blocks
+    const int KS = tc_plan(t.N, t.K, t.m_max, t.epi == EPI_SWIGLU, t.scratch != nullptr, &d.kb_per_cta);
     d.mtiles = mtiles;
     dim3 grid(tiles * mtiles, KS, 1);
     cudaError_t e;
