@@ -108,7 +108,7 @@ struct sagc_model {
     std::vector<TcMap> wmaps;                  // per layer: q k v o g u d ; last = lm_head
     std::vector<TcMap> kvmaps;                 // per layer: the KV pool as a 2-D tensor (tcgen05 decode attention)
     void* pfmaps_d; int pf_on; long long pf_budget;   // SAGC_PF (default 0, measured slower): every decode kernel prefetches the next GEMM's leading weight blocks into L2
-    int att_tc, att_tc_stages;                 // SAGC_ATT_TC (default 1): decode attention on tcgen05; ring depth (0 = deepest)
+    int att_tc, att_tc_stages;                 // SAGC_ATT_TC (default 1 at head_dim 128; 2 = on every decode step, 0 = never): decode attention on tcgen05; ring depth (0 = deepest)
     TcMap amaps[3][4];                         // {xs, att_s, act_s} x UMMA N {32, 64, 128, 256}
     // persistent decode-step kernel (decode_step.cu): static work plan, device copies of the per-layer tables, counters
     bool step_ok; int n_sm, step_slots, gbar_n, tcnt_n, tiles_per_layer;
@@ -219,7 +219,7 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     }
     // measured (profiles/r02_attention.md): the tcgen05 kernel wins at head_dim 128 (7B shape: 1.3 - 1.6x in the tail, 1.35x at 256
     // rows); at head_dim 64 its per-tile gain does not pay for its longer prologue / epilogue at the short contexts of those models
-    m->att_tc = env_int("SAGC_ATT_TC", c.head_dim == 128 ? 1 : 0) && attention_tc_supports(c.head_dim, c.page_tokens, c.n_q_heads / c.n_kv_heads);
+    m->att_tc = attention_tc_supports(c.head_dim, c.page_tokens, c.n_q_heads / c.n_kv_heads) ? env_int("SAGC_ATT_TC", c.head_dim == 128 ? 1 : 0) : 0;
     m->att_tc_stages = env_int("SAGC_ATT_TC_STAGES", 0);
     if (m->att_tc) {
         m->kvmaps.resize(L > 0 ? L : 1);
@@ -378,9 +378,10 @@ static int pick_kind(const sagc_model* m, int path, int m_max) {
 static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cudaStream_t st);
 
 // layers only (x ends up holding the final residual stream).  Returns kernels launched or <0.
-static int enqueue_layers(sagc_model* m, const RowSet& rs, int n_splits, int kind, cudaStream_t st) {
+static int enqueue_layers(sagc_model* m, const RowSet& rs, int n_splits_enc, int kind, cudaStream_t st) {
+    const int n_splits = n_splits_enc & 0xfff;
     const sagc_model_config& c = m->cfg;
-    if (kind == LIN_TC) return enqueue_layers_tc(m, rs, n_splits, st);
+    if (kind == LIN_TC) return enqueue_layers_tc(m, rs, n_splits_enc, st);
     int n = 0, r;
 #define LAUNCH(expr) do { r = (expr); if (r < 0) return -1; n += r; } while (0)
     const int skip = m->skip_mask;
@@ -434,7 +435,9 @@ static int enqueue_layers(sagc_model* m, const RowSet& rs, int n_splits, int kin
 
 // tcgen05 variant of the layer stack: activations travel between kernels as pre-split bf16 rows
 // (xs / att_s / act_s), the RMSNorm gain is folded in by the producer and 1/rms by the consumer.
-static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cudaStream_t st) {
+static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits_enc, cudaStream_t st) {
+    const bool att_tc_step = (n_splits_enc & 0x1000) != 0;
+    const int n_splits = n_splits_enc & 0xfff;
     const sagc_model_config& c = m->cfg;
     int n = 0, r;
     const int skip = m->skip_mask;
@@ -491,7 +494,7 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits, cuda
         const TcPf pf_gu = make_pf((size_t)l * 7 + 4, 2, c.d_ff / 128, c.d_ff / 128, 0, c.d_ff, c.d_model, true);   // -> gate / up
         if (m->pf_on & 2) aa.pf = pf_gu;
         if (!(skip & 1)) {
-            if (fuse_att && m->att_tc) LAUNCH(launch_attention_tc(aa, &m->kvmaps[l], m->att_tc_stages, st));
+            if (fuse_att && m->att_tc && att_tc_step) LAUNCH(launch_attention_tc(aa, &m->kvmaps[l], m->att_tc_stages, st));
             else LAUNCH(launch_attention(aa, st));
         }
 
@@ -573,6 +576,7 @@ static int round_bucket(int live) {
     return ((live + 63) / 64) * 64;
 }
 
+static constexpr int ATT_TC_FLAG = 0x1000;      // pick_splits: this step's attention runs on the tcgen05 kernel
 static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
     const int ctas = m_bucket * m->cfg.n_kv_heads;
     const int target = (3 * sagc::g_num_sms) / 2;
@@ -586,7 +590,10 @@ static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
     while (s * 2 <= want) s *= 2;
     const int smax = 8;                       // <= 8 splits merge inside a cluster (attention.cu)
     if (s > smax) s = smax;
-    if (m->att_tc && m->cfg.head_dim >= 64) {
+    // The tcgen05 kernel pays ~4 us more prologue / epilogue / L2 merge than the register-HMMA unit and streams a tile in half
+    // the time: it wins from ~2 000 cached tokens per row, or at any context once the grid is large (256 rows x 1 100 tokens:
+    // 104 vs 159 us); with few rows at ~1 000 tokens it loses (19.5 vs 17.1 us).  The choice travels in bit 12 of the split count.
+    if (m->att_tc && m->cfg.head_dim >= 64 && (m_bucket >= 32 || ctx_bound >= 2048 || m->att_tc > 1)) {
         // tcgen05 decode attention: one CTA per SM (the K/V ring fills shared memory), >= 2 tiles of 128 tokens per
         // split, partials merged through L2 by the last arriver; more than 16 splits cost more in the merge than they
         // save in the scan (1 row x 16 000 tokens: 26 us with 16 splits, 30 us with 32)
@@ -597,6 +604,7 @@ static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
         if (w2 > m->max_splits) w2 = m->max_splits;
         s = 1;
         while (s * 2 <= w2) s *= 2;
+        s |= ATT_TC_FLAG;
     }
     return s;
 }

@@ -204,3 +204,49 @@ def test_paged_attention_long_context(B, Hq, Hkv, hd, splits, variant):
     q, kv, pt, ref = _attention_case(rng, ctxs, Hq, Hkv, hd, 64)
     out = B.debug_attention(_dev(q), _dev(kv.view(np.int16)), _dev(pt), _dev(ctxs), Hq, Hkv, hd, 64, splits, variant).cpu().numpy()
     assert np.max(np.abs(out - ref)) < 2e-5, np.max(np.abs(out - ref))
+
+
+BENCH_SHAPES = {   # the attention launches of the timed decode steps (bench.py phases), by model shape: (contexts, Hq, Hkv, hd)
+    "7b_tail1": (np.array([16000]), 28, 4, 128),
+    "7b_tail8": (np.array([3000, 2500, 3500, 2800, 5000, 2000, 2200, 4100]), 28, 4, 128),
+    "7b_full": (1100 + (np.arange(256) * 37) % 600, 28, 4, 128),
+    "c2_tail8": (np.array([2000, 1500, 3000, 1200, 4100, 900, 2500, 1800]), 14, 2, 64),
+    "c2_full": (300 + (np.arange(512) * 13) % 300, 14, 2, 64),
+}
+
+
+@pytest.mark.parametrize("name,variant,splits", [("7b_tail1", 0, 8), ("7b_tail1", 2, 16), ("7b_tail8", 0, 4), ("7b_tail8", 2, 4),
+                                                 ("7b_full", 0, 1), ("7b_full", 2, 1), ("c2_tail8", 0, 8), ("c2_tail8", 2, 8),
+                                                 ("c2_full", 0, 1), ("c2_full", 2, 1)])
+def test_paged_attention_bench_shapes(B, name, variant, splits):
+    """Parity in the launch configurations the bench times (rows x kv heads x splits of the FULL and TAIL phases of the
+    0.5B and 7B shapes), both attention kernels; fp64 definition on every row (<= 8 rows) or on 8 seeded rows.
+    (Also the committed command behind profiles/r02_attention.md.)"""
+    ctxs, Hq, Hkv, hd = BENCH_SHAPES[name]
+    ctxs = ctxs.astype(np.int32)
+    page, M, r = 64, len(ctxs), Hq // Hkv
+    rng = np.random.default_rng(len(name) + hd)
+    nb = (ctxs + page - 1) // page
+    n_pages = int(nb.sum()) + 1
+    g = torch.Generator(device="cuda").manual_seed(7)
+    kv = torch.randn((n_pages, 2, Hkv, page, hd), device="cuda", generator=g).to(torch.bfloat16)
+    perm = rng.permutation(n_pages).astype(np.int32)
+    pt = -np.ones((M, int(nb.max())), dtype=np.int32)
+    k = 0
+    for m in range(M):
+        pt[m, :nb[m]] = perm[k:k + nb[m]]
+        k += int(nb[m])
+    q = rng.standard_normal((M, Hq, hd)).astype(np.float32)
+    out = B.debug_attention(_dev(q), kv.view(torch.int16), _dev(pt), _dev(ctxs), Hq, Hkv, hd, page, splits, variant).cpu().numpy()
+    rows = range(M) if M <= 8 else sorted(rng.choice(M, size=8, replace=False))
+    worst = 0.0
+    for m in rows:
+        c = int(ctxs[m])
+        pages = kv[torch.from_numpy(pt[m, :nb[m]].astype(np.int64)).cuda()].double().cpu().numpy()      # [nb][2][Hkv][page][hd]
+        K = pages[:, 0].transpose(1, 0, 2, 3).reshape(Hkv, -1, hd)[:, :c]
+        V = pages[:, 1].transpose(1, 0, 2, 3).reshape(Hkv, -1, hd)[:, :c]
+        for h in range(Hq):
+            sc = K[h // r] @ q[m, h].astype(np.float64) / np.sqrt(hd)
+            p = np.exp(sc - sc.max())
+            worst = max(worst, float(np.max(np.abs(out[m, h] - (p / p.sum()) @ V[h // r]))))
+    assert worst < 2e-5, worst

@@ -297,18 +297,23 @@ def test_config2_truncated(B, monkeypatch, variant):
     _sampled_parity(B, 2, 2, 256, 8, 14, fl, 0)
 
 
-@pytest.mark.parametrize("step_kernel", [0, 1])
-def test_config3_truncated(B, monkeypatch, step_kernel):
-    """1.5B shape (head_dim 128, r = 6, DAPO config): 1 prompt x 96 tokens (ragged vs the 64-token page) x G=16."""
+@pytest.mark.parametrize("step_kernel,att_tc", [(0, 0), (0, 2), (1, 0)])
+def test_config3_truncated(B, monkeypatch, step_kernel, att_tc):
+    """1.5B shape (head_dim 128, r = 6, DAPO config): 1 prompt x 96 tokens (ragged vs the 64-token page) x G=16.
+    att_tc = 2 forces the tcgen05 attention kernel at these short contexts too (by default it takes the steps with
+    >= 32 live rows or >= 2 048 cached tokens), 0 = the register-HMMA unit on every step."""
     monkeypatch.setenv("SAGC_STEP", str(step_kernel))
+    monkeypatch.setenv("SAGC_ATT_TC", str(att_tc))
     fl = np.array([10, 3, 10, 10, 1, 10, 7, 10, 10, 10, 5, 10, 10, 2, 10, 10], dtype=np.int32)
     _sampled_parity(B, 3, 1, 96, 16, 10, fl, 0, n_dump_seq=2)
 
 
-@pytest.mark.parametrize("cfg,G", [(4, 32)])
-def test_config4_truncated(B, cfg, G):
+@pytest.mark.parametrize("cfg,G,att_tc", [(4, 32, 1), (4, 32, 2), (4, 32, 0)])
+def test_config4_truncated(B, monkeypatch, cfg, G, att_tc):
     """7B shape (configs 4 and 5 share it): 1 prompt x 128 tokens x G=32 -> 32 live rows on the tcgen05 path,
-    then the tail path; logits of two sampled sequences against the fp32 oracle."""
+    then the tail path; logits of two sampled sequences against the fp32 oracle.  att_tc: 1 = default policy (tcgen05
+    attention while 32 rows are live, register-HMMA below), 2 = tcgen05 attention on every step, 0 = never."""
+    monkeypatch.setenv("SAGC_ATT_TC", str(att_tc))
     fl = np.array([6, 4, 6, 3, 6, 2, 6, 1, 6, 4, 6, 3] + [1, 2, 3, 4] * 5, dtype=np.int32)   # 6 live in steps 5-6
     _sampled_parity(B, cfg, 1, 128, G, 6, fl, 0, n_dump_seq=2)
 
