@@ -2,6 +2,7 @@
 // (activation row, kv head, K-split).  Serves prefill (every prompt position is a row with ctx = position + 1),
 // head_dim 32, decode steps with more than 64 live rows and the sagc_debug_attention parity entry; decode steps
 // with <= 64 live rows run the same unit inside the persistent decode-step kernel (decode_step.cu).
+#include <cstdlib>
 #include "attention_body.cuh"
 
 namespace sagc {
@@ -32,8 +33,16 @@ __global__ void __launch_bounds__(ATT_THREADS) k_attention(AttnArgs a) {
 
 template <int HD, int WARPS, int NSTAGE>
 static int launch_att_geom(const AttnArgs& a, cudaStream_t st) {
-    constexpr int BYTES = AttGeom<HD, WARPS, NSTAGE>::BYTES;
-    if (cudaFuncSetAttribute(k_attention<HD, WARPS, NSTAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, BYTES) != cudaSuccess) return -1;
+    constexpr int RING = AttGeom<HD, WARPS, NSTAGE>::BYTES;
+    // Decode: ask for at least 114 KB, so that the CTAs of the NEXT kernel (the O projection, 113 KB each, launched early by
+    // PDL) cannot become resident beside an attention CTA.  Co-resident successors fill their weight ring early, but they take
+    // issue slots and shared-memory bandwidth from the kernel on the critical path: measured on one box, 0.5B shape, FULL / MID /
+    // TAIL ms per step 1.098 / 0.945 / 0.876 with the bare 96 KB ring, 1.057 / 0.927 / 0.871 with 114 KB (120 KB: the same).
+    // (Round 1's kernel had 25 KB of static shared memory on top of the ring and was never co-resident; the refactoring of round 2
+    // that overlaid those buffers on the ring cost 3.7 % of FULL until this was found.)
+    static const int pad_kb = [] { const char* e = getenv("SAGC_ATT_PAD_KB"); return e ? atoi(e) : 114; }();
+    const int BYTES = (a.prefetch && RING < pad_kb * 1024) ? pad_kb * 1024 : RING;
+    if (cudaFuncSetAttribute(k_attention<HD, WARPS, NSTAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, BYTES > RING ? BYTES : RING) != cudaSuccess) return -1;
     dim3 grid(a.m_max, a.Hkv, a.n_splits);
     if (a.n_splits > 1 && a.n_splits <= 8) {      // 2..8 splits merge inside a cluster through DSMEM
         AttnArgs ac = a;

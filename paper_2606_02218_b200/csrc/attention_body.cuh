@@ -50,8 +50,9 @@ __device__ __forceinline__ void store_out(const AttnArgs& a, int row, int col, f
 
 // element(s) of the activation row that holds q | k | v: fp32, or 64-bit fixed point * 2^-32 * (1/rms of the row)
 static constexpr float ATT_FX_SCALE = 2.3283064365386963e-10f;      // 2^-32
+template <bool FX = true>
 __device__ __forceinline__ void att_load8(const AttnArgs& a, int row, size_t col, float rs, float (&o)[8]) {
-    if (a.q_fx != nullptr) {
+    if (FX && a.q_fx != nullptr) {
         const longlong2* p = reinterpret_cast<const longlong2*>(a.q_fx + (size_t)row * a.ldq + col);
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -65,8 +66,9 @@ __device__ __forceinline__ void att_load8(const AttnArgs& a, int row, size_t col
         o[0] = x0.x; o[1] = x0.y; o[2] = x0.z; o[3] = x0.w; o[4] = x1.x; o[5] = x1.y; o[6] = x1.z; o[7] = x1.w;
     }
 }
+template <bool FX = true>
 __device__ __forceinline__ float att_load1(const AttnArgs& a, int row, size_t col, float rs) {
-    if (a.q_fx != nullptr) return __ll2float_rn(__ldcg(a.q_fx + (size_t)row * a.ldq + col)) * ATT_FX_SCALE * rs;
+    if (FX && a.q_fx != nullptr) return __ll2float_rn(__ldcg(a.q_fx + (size_t)row * a.ldq + col)) * ATT_FX_SCALE * rs;
     return __ldcg(a.q + (size_t)row * a.ldq + col);
 }
 
@@ -149,31 +151,23 @@ __device__ __forceinline__ void attention_unit(const AttnArgs& a, const int row,
     // K chunk c of token j -> chunk c ^ ksw(j); V chunk c -> c ^ vsw(j)   (bank-conflict free)
     auto ksw = [](int j) { return CPR >= 8 ? ((j & 1) << 2) : 0; };
     auto vsw = [](int j) { return CPR >= 8 ? (j & 7) : ((j >> 1) & 3); };
-    // Tile loader.  Thread -> (token row j0 + k * RPT, 16-byte chunk `part`), k = 0 .. NPASS-1: the chunk, the swizzled
-    // shared-memory offsets and the per-head base pointer are per-thread constants (RPT is a multiple of 16, so the
-    // swizzle terms do not depend on k); a pass costs one page lookup, one 64-bit multiply-add and two cp.async.
-    // (The address arithmetic was 55 % of the kernel's instructions before: profiles/r02_attention.md.)
-    constexpr int RPT = ATT_THREADS / CPR;       // token rows covered per pass
-    constexpr int NPASS = ATT_TILE / RPT;
-    static_assert(ATT_TILE % RPT == 0 && RPT % 16 == 0, "tile / thread mapping of the K/V loader");
-    const int ld_part = tid % CPR, ld_j0 = tid / CPR;
-    const uint32_t ld_ks = (uint32_t)ld_j0 * ROWB + (uint32_t)((ld_part ^ ksw(ld_j0)) << 4);
-    const uint32_t ld_vs = (uint32_t)(ATT_TILE + ld_j0) * ROWB + (uint32_t)((ld_part ^ vsw(ld_j0)) << 4);
-    const size_t ld_pstride = (size_t)2 * a.Hkv * head_stride;                      // elements per page (K and V, all kv heads)
-    const bf16_t* ld_base = a.kv_layer + (size_t)kvh * head_stride + ld_part * 8;   // K of this kv head; V sits Hkv slabs further
-    const size_t ld_voff = (size_t)a.Hkv * head_stride;
+    // Tile loader: 16-byte chunk c of the tile -> (token j = c / CPR, part = c % CPR).  (A variant with per-thread-constant
+    // chunk / swizzle / base pointer -- 45 % fewer loader instructions -- measured 0.5 us SLOWER per launch at 64 rows x 2 kv heads.)
     auto load_tile = [&](int tile, int stage) {
         unsigned char* base = kv_s + (size_t)stage * G::STAGE;
-        const int tok0 = t_begin + tile * ATT_TILE + ld_j0;
+        const int t0 = t_begin + tile * ATT_TILE;
 #pragma unroll
-        for (int k = 0; k < NPASS; ++k) {
-            const int tok = tok0 + k * RPT;
-            int pg = -1;
-            if (tok < t_end) pg = pg_cached ? sm->pg_s[(tok >> pshift) - b_begin] : pt[tok >> pshift];
+        for (int c = tid; c < ATT_TILE * CPR; c += ATT_THREADS) {
+            const int j = c / CPR, part = c % CPR;
+            const int tok = t0 + j;
+            const int blk = tok >> pshift;
+            const int pg = (tok < t_end) ? (pg_cached ? sm->pg_s[blk - b_begin] : pt[blk]) : -1;
             const bool ok = pg >= 0;             // masked tail, or an unmapped block after a pool-exhaustion error: zero fill
-            const bf16_t* kp = ld_base + (ok ? (size_t)pg * ld_pstride + (size_t)((tok & pmask) * HD) : (size_t)0);
-            cp_async16(base + ld_ks + (uint32_t)(k * RPT * ROWB), kp, ok ? 16 : 0);
-            cp_async16(base + ld_vs + (uint32_t)(k * RPT * ROWB), kp + ld_voff, ok ? 16 : 0);
+            const bf16_t* kp = a.kv_layer + ((size_t)(ok ? pg : 0) * 2 * a.Hkv + kvh) * head_stride +
+                               (size_t)(ok ? (tok & pmask) : 0) * HD + part * 8;
+            const bf16_t* vp = kp + (size_t)a.Hkv * head_stride;
+            cp_async16(base + (size_t)j * ROWB + ((part ^ ksw(j)) << 4), kp, ok ? 16 : 0);
+            cp_async16(base + (size_t)(ATT_TILE + j) * ROWB + ((part ^ vsw(j)) << 4), vp, ok ? 16 : 0);
         }
     };
     // fused RoPE (decode): cos/sin of this row's position for the q fragments, fetched before the wait
@@ -211,13 +205,13 @@ __device__ __forceinline__ void attention_unit(const AttnArgs& a, const int row,
     uint32_t knew = 0, vnew = 0;                    // designated unit: bf16 bits of the new k pair / v element
     {
         const float scale = rsqrtf((float)HD);
-        const float rs = a.q_fx != nullptr ? __ldcg(a.q_rstd + row) : 1.f;
+        const float rs = (MEGA && a.q_fx != nullptr) ? __ldcg(a.q_rstd + row) : 1.f;      // the fixed-point q source exists in the decode-step kernel only
         const size_t qcol = (size_t)(kvh * r + g) * HD + 8 * q;
         float xq[KB][8];
 #pragma unroll
         for (int kb = 0; kb < KB; ++kb) {
             if (g < r) {
-                att_load8(a, row, qcol + kb * 32, rs, xq[kb]);
+                att_load8<MEGA>(a, row, qcol + kb * 32, rs, xq[kb]);
             } else {
 #pragma unroll
                 for (int e = 0; e < 8; ++e) xq[kb][e] = 0.f;
@@ -228,10 +222,10 @@ __device__ __forceinline__ void attention_unit(const AttnArgs& a, const int row,
             const size_t kcol = (size_t)a.Hq * HD + (size_t)kvh * HD;
             const size_t vcol = kcol + (size_t)a.Hkv * HD;
             if (tid < HD / 2) {
-                const float k0 = att_load1(a, row, kcol + tid, rs), k1 = att_load1(a, row, kcol + tid + HD / 2, rs);
+                const float k0 = att_load1<MEGA>(a, row, kcol + tid, rs), k1 = att_load1<MEGA>(a, row, kcol + tid + HD / 2, rs);
                 knew = f32_to_bf16_bits(k0 * kcs.x - k1 * kcs.y) | (f32_to_bf16_bits(k1 * kcs.x + k0 * kcs.y) << 16);
             }
-            if (tid < HD) vnew = f32_to_bf16_bits(att_load1(a, row, vcol + tid, rs));
+            if (tid < HD) vnew = f32_to_bf16_bits(att_load1<MEGA>(a, row, vcol + tid, rs));
         }
         if (fuse) {
 #pragma unroll
@@ -331,10 +325,8 @@ __device__ __forceinline__ void attention_unit(const AttnArgs& a, const int row,
         ls += __shfl_xor_sync(0xffffffffu, ls, 2);
         l_run = l_run * f + ls;
         m_run = m_new;
-        if (__any_sync(0xffffffffu, f != 1.f)) {     // running max unchanged on every lane: f == 1 exactly, skip the rescale
 #pragma unroll
-            for (int n = 0; n < NT; ++n) { o[n][0] *= f; o[n][1] *= f; o[n][2] *= f; o[n][3] *= f; }
-        }
+        for (int n = 0; n < NT; ++n) { o[n][0] *= f; o[n][1] *= f; o[n][2] *= f; o[n][3] *= f; }
         // P as the A operand: rows g = hi, rows g+8 = lo; k = 16 tokens
         uint32_t pa[4];
         split2(p[0], p[1], pa[0], pa[1]);

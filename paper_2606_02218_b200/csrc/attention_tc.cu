@@ -211,10 +211,6 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
 
     if (warp == 0) {
         // ===== TMA producer =====================================================================
-        // attention is latency-bound: the next GEMM's leading weight blocks travel to L2 meanwhile (see TcPf)
-        if (lane == 0) tc_prefetch_next(a.pf, ((int)blockIdx.z * (int)gridDim.y + (int)blockIdx.y) * (int)gridDim.x + (int)blockIdx.x,
-                                        (int)(gridDim.x * gridDim.y * gridDim.z));
-        __syncwarp();
         if (n_tiles > 0) {                                       // all 32 lanes, converged
             const int ppt = ATC_TILE >> pshift;                  // pages per tile
             const uint32_t box_bytes = (uint32_t)a.page * 128u;

@@ -53,13 +53,6 @@ struct RopeArgs {
 int launch_rope_append(const RopeArgs& a, cudaStream_t st);
 
 // Paged GQA attention over ragged contexts with split-K + in-kernel LSE merge.  Step a7.
-struct TcPf {
-    const void* maps;       // device CUtensorMap[n_maps], consecutive, box 64 x 128 (null = off)
-    int n_maps;
-    int tiles[3];           // 128-row tiles of each map
-    int ks, kbpc, nkb;      // next kernel: K-split ranks, 64-wide k blocks per rank, leading blocks to fetch per (tile, rank)
-};
-
 struct AttnArgs {
     const float* q;         // [M][ldq] (first Hq*hd columns are the rotated queries)
     int ldq;
@@ -84,7 +77,6 @@ struct AttnArgs {
     const long long* q_fx; const float* q_rstd;
     int prefetch;           // 1 in decode: cached positions older than the newest one predate the upstream kernel
     int cluster_merge;      // set by the launcher: the n_splits CTAs of a (row, kv head) form a cluster and merge through DSMEM
-    TcPf pf;                // attention_tc.cu: L2 prefetch of the next GEMM's leading weight blocks (maps == null: off)
     unsigned long long* dbg; // attention_tc.cu built with -DSAGC_ATT_TIMELINE: clock64 stamps of CTA (0,0,0), [role 4][tile 64][event 8]; else unused
 };
 int launch_attention(const AttnArgs& a, cudaStream_t st);
@@ -173,7 +165,6 @@ struct TcLinearArgs {
     int K, N;                   // N = output rows (EPI_SWIGLU: d_ff)
     const int* m_dev; int m_max;
     int epi;
-    TcPf pf;                    // L2 prefetch of the NEXT GEMM's leading weight blocks, issued after this kernel's own loads (maps == null: off)
     float* Y; int ldy; const float* R;
     bf16_t* xs_out; int ld_xs; const bf16_t* norm_next; float* ssq_out;
     const float* ssq_in; int ssq_in_tiles; int ssq_ld; float eps; int k_norm;

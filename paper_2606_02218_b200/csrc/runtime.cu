@@ -107,7 +107,6 @@ struct sagc_model {
     int ssq_ld, d_tiles;
     std::vector<TcMap> wmaps;                  // per layer: q k v o g u d ; last = lm_head
     std::vector<TcMap> kvmaps;                 // per layer: the KV pool as a 2-D tensor (tcgen05 decode attention)
-    void* pfmaps_d; int pf_on; long long pf_budget;   // SAGC_PF (default 0, measured slower): every decode kernel prefetches the next GEMM's leading weight blocks into L2
     int att_tc, att_tc_stages;                 // SAGC_ATT_TC (default 1 at head_dim 128; 2 = on every decode step, 0 = never): decode attention on tcgen05; ring depth (0 = deepest)
     TcMap amaps[3][4];                         // {xs, att_s, act_s} x UMMA N {32, 64, 128, 256}
     // persistent decode-step kernel (decode_step.cu): static work plan, device copies of the per-layer tables, counters
@@ -209,7 +208,6 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
     m->h_prompt_cap = m->h_tok_cap = m->h_len_cap = m->h_grp_cap = 0;
     m->score_logits = nullptr; m->score_cap = 0; m->seq_off_d = nullptr; m->seq_off_cap = 0;
     m->step_ok = false; m->n_sm = 0; m->step_trace = nullptr;
-    m->pfmaps_d = nullptr; m->pf_on = 0; m->pf_budget = 0;
 
     DA(m->kv_pool, m->layer_stride * (size_t)(L > 0 ? L : 1));
     // finite everywhere: a masked position of a partially filled page meets p = 0 in the tcgen05 attention (0 * NaN would not be 0)
@@ -305,17 +303,6 @@ extern "C" int sagc_model_create(const sagc_model_config* cfg, const sagc_weight
                 bad |= tc_make_map(&m->amaps[2][i], m->act_s, 2 * (long long)Rp, c.d_ff, 32 << i);
             }
             if (bad) { sagc_model_destroy(m); return set_err(SAGC_ECUDA, "cuTensorMapEncodeTiled failed"); }
-            // device copy of the weight maps for the cross-kernel L2 prefetch (TcPf)
-            // Experiment knob, OFF: measured slower on both shapes however the prefetch is timed (cfg2 TAIL 0.88 -> 0.99 ms per step with
-            // the prefetch issued after the producer's last load, -> 1.07 ms after the last MMA; 7B TAIL 4.16 -> 4.36 ms).  bit 1 = also from attention.
-            m->pf_on = env_int("SAGC_PF", 0);
-            m->pf_budget = (long long)env_int("SAGC_PF_MB", 40) << 20;
-            if (m->pf_on) {
-                unsigned char* pm = nullptr;
-                DA(pm, m->wmaps.size() * sizeof(TcMap));
-                m->pfmaps_d = pm;
-                CU(cudaMemcpy(m->pfmaps_d, m->wmaps.data(), m->wmaps.size() * sizeof(TcMap), cudaMemcpyHostToDevice));
-            }
         }
         // persistent decode-step kernel: one CTA per SM, static unit -> CTA plan, tensor maps / norm gains in device tables
         m->step_ok = false; m->wmaps_d = nullptr; m->plan_d = nullptr; m->norm1_d = m->norm2_d = nullptr; m->step_sync = nullptr; m->step_err = nullptr;
@@ -443,20 +430,6 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits_enc, 
     const int skip = m->skip_mask;
     const int qd = c.n_q_heads * c.head_dim, kvd = c.n_kv_heads * c.head_dim;
     const int nbi = tc_nb_index(rs.m_max);
-    // cross-kernel L2 prefetch (decode only): descriptor of the NEXT GEMM's weight streams for each kernel of the layer
-    const bool pf_on = m->pf_on && m->pfmaps_d != nullptr && rs.m_dev != nullptr;
-    auto make_pf = [&](size_t first_map, int n_maps, int t0, int t1, int t2, int N, int K, bool swiglu) {
-        TcPf pf = {};
-        if (!pf_on) return pf;
-        pf.maps = reinterpret_cast<const TcMap*>(m->pfmaps_d) + first_map;
-        pf.n_maps = n_maps; pf.tiles[0] = t0; pf.tiles[1] = t1; pf.tiles[2] = t2;
-        pf.ks = tc_plan(N, K, rs.m_max, swiglu, m->tc_scratch != nullptr, &pf.kbpc);
-        const long long streams = (long long)(t0 + t1 + t2) * pf.ks;
-        long long nkb = m->pf_budget / (streams * 16384);      // one box = 128 rows x 64 bf16
-        if (nkb > pf.kbpc) nkb = pf.kbpc;
-        pf.nkb = (int)nkb;
-        return pf;
-    };
     LAUNCH(launch_embed_split(m->embed, rs.tok, rs.m_dev, rs.m_max, c.d_model, m->x, m->norm1[0], m->xs, m->ssq,
                               m->ssq_ld, m->d_tiles, st));
     for (int l = 0; l < c.n_layers; ++l) {
@@ -472,7 +445,6 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits_enc, 
         t.max_blocks = m->max_blocks; t.page = c.page_tokens; t.Hkv = c.n_kv_heads; t.hd = c.head_dim; t.q_rows = qd; t.kv_rows = kvd;
         const bool fuse_rope = false;          // RoPE + append in the QKV epilogue (EPI_QKV): measured -4% in FULL, kept off
         if (!fuse_rope) t.epi = EPI_STORE;
-        t.pf = make_pf((size_t)l * 7 + 3, 1, c.d_model / 128, 0, 0, c.d_model, qd, false);                       // -> O
         if (!(skip & 4)) LAUNCH(launch_linear_tc(t, st));
         // decode: RoPE + KV append are done inside the attention kernel (one launch less per layer)
         const bool fuse_att = !fuse_rope && rs.m_dev != nullptr && c.head_dim >= 64;
@@ -491,8 +463,6 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits_enc, 
         aa.n_splits = n_splits; aa.part_o = m->part_o; aa.part_ml = m->part_ml; aa.counters = m->counters;
         aa.out = m->att; aa.prefetch = (rs.m_dev != nullptr) ? 1 : 0; aa.out_split = m->att_s; aa.ld_split = qd;
         aa.fuse_rope = fuse_att ? 1 : 0; aa.rope_cs = m->rope_cs; aa.row_pos = rs.pos; aa.kv_layer_w = kv_layer;
-        const TcPf pf_gu = make_pf((size_t)l * 7 + 4, 2, c.d_ff / 128, c.d_ff / 128, 0, c.d_ff, c.d_model, true);   // -> gate / up
-        if (m->pf_on & 2) aa.pf = pf_gu;
         if (!(skip & 1)) {
             if (fuse_att && m->att_tc && att_tc_step) LAUNCH(launch_attention_tc(aa, &m->kvmaps[l], m->att_tc_stages, st));
             else LAUNCH(launch_attention(aa, st));
@@ -503,7 +473,6 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits_enc, 
         o.m_dev = rs.m_dev; o.m_max = rs.m_max; o.epi = EPI_RESID; o.Y = m->x; o.R = m->x; o.ldy = c.d_model;
         o.xs_out = m->xs; o.ld_xs = c.d_model; o.norm_next = m->norm2[l]; o.ssq_out = m->ssq; o.ssq_ld = m->ssq_ld;
         o.eps = c.rms_eps; o.pdl = m->use_pdl; o.scratch = m->tc_scratch;
-        o.pf = pf_gu;                                                                                             // -> gate / up
         if (!(skip & 4)) LAUNCH(launch_linear_tc(o, st));
 
         TcLinearArgs gu = {};
@@ -511,7 +480,6 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits_enc, 
         gu.b = &m->amaps[0][nbi]; gu.K = c.d_model; gu.N = c.d_ff; gu.m_dev = rs.m_dev; gu.m_max = rs.m_max;
         gu.epi = EPI_SWIGLU; gu.xs_out = m->act_s; gu.ld_xs = c.d_ff; gu.ssq_in = m->ssq; gu.ssq_in_tiles = m->d_tiles;
         gu.ssq_ld = m->ssq_ld; gu.eps = c.rms_eps; gu.k_norm = c.d_model; gu.pdl = m->use_pdl; gu.scratch = m->tc_scratch;
-        gu.pf = make_pf((size_t)l * 7 + 6, 1, c.d_model / 128, 0, 0, c.d_model, c.d_ff, false);                 // -> down
         if (!(skip & 4)) LAUNCH(launch_linear_tc(gu, st));
 
         TcLinearArgs dn = {};
@@ -519,15 +487,6 @@ static int enqueue_layers_tc(sagc_model* m, const RowSet& rs, int n_splits_enc, 
         dn.m_dev = rs.m_dev; dn.m_max = rs.m_max; dn.epi = EPI_RESID; dn.Y = m->x; dn.R = m->x; dn.ldy = c.d_model;
         dn.xs_out = m->xs; dn.ld_xs = c.d_model; dn.norm_next = (l + 1 < c.n_layers) ? m->norm1[l + 1] : m->final_norm;
         dn.ssq_out = m->ssq; dn.ssq_ld = m->ssq_ld; dn.eps = c.rms_eps; dn.pdl = m->use_pdl; dn.scratch = m->tc_scratch;
-        if (l + 1 < c.n_layers) {
-            dn.pf = make_pf((size_t)(l + 1) * 7, 3, qd / 128, kvd / 128, kvd / 128, m->Nqkv, c.d_model, false);  // -> next layer's QKV
-        } else if (pf_on) {             // -> LM head: the first vocabulary tile of each of its persistent CTAs
-            const int vt = c.vocab / 128 < sagc::g_num_sms ? c.vocab / 128 : sagc::g_num_sms;
-            dn.pf.maps = reinterpret_cast<const TcMap*>(m->pfmaps_d) + (size_t)c.n_layers * 7;
-            dn.pf.n_maps = 1; dn.pf.tiles[0] = vt; dn.pf.ks = 1; dn.pf.kbpc = c.d_model / 64;
-            long long nkb = m->pf_budget / ((long long)vt * 16384);
-            dn.pf.nkb = (int)(nkb > dn.pf.kbpc ? dn.pf.kbpc : nkb);
-        }
         if (!(skip & 4)) LAUNCH(launch_linear_tc(dn, st));
     }
     return n;

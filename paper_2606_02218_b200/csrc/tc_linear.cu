@@ -40,7 +40,6 @@ struct TcDev {
     const float* ssq_in; int ssq_in_tiles;   // fused RMSNorm of the INPUT: rstd[m] from these partials
     int ssq_ld; float eps; int k_norm;
     int stages;                     // smem ring depth chosen by the launcher
-    TcPf pf;                        // next GEMM's weight streams to prefetch into L2
     int mtiles;                     // batch tiles of MB rows; blockIdx.x = weight tile * mtiles + batch tile
     float* scratch;                 // split-K partial tiles [cta][NA][MB][128] (L2-resident), KS > 1 only
     // EPI_QKV (fused RoPE + KV append)
@@ -279,8 +278,9 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     // the batch tiles of one weight tile are NEIGHBOURS in launch order: they run in the same wave, so the weight tile
     // comes from DRAM once and the other batch tiles hit L2 (with batch tiles in grid.z every wave re-read the matrix:
     // dram__bytes_read was 2x the weights at 256 rows, profiles/r02_ncu_top_kernels.md)
-    const int tile = (int)blockIdx.x / a.mtiles, row0 = tile * 128;
-    const int m0 = ((int)blockIdx.x % a.mtiles) * MB;
+    // (decode steps with <= 128 rows have ONE batch tile: no division on their prologue path)
+    const int tile = a.mtiles == 1 ? (int)blockIdx.x : (int)blockIdx.x / a.mtiles, row0 = tile * 128;
+    const int m0 = a.mtiles == 1 ? 0 : ((int)blockIdx.x % a.mtiles) * MB;
     const int cta_id = (int)blockIdx.x * KS + rank;
     const int kb0 = rank * a.kb_per_cta;
     const int nk = max(0, min(a.n_kb, kb0 + a.kb_per_cta) - kb0);
@@ -362,9 +362,6 @@ k_linear_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             }
             __syncwarp();
         }
-        // every MMA of this CTA is issued, so its weight stream has landed: from here to the next kernel's first loads the
-        // bus would idle (epilogue, cluster reduction, the next prologue) -- fetch the next GEMM's leading blocks into L2
-        if (lane == 0) tc_prefetch_next(a.pf, cta_id, (int)gridDim.x * KS);
     } else {
         // ===== epilogue warps: TMEM -> (hi + lo) -> shared reduce buffer =====
         const int lg = warp & 3;                      // TMEM lane group of this warp
@@ -498,6 +495,8 @@ static cudaError_t launch_tc_inst(const TcLinearArgs& t, const TcDev& d, dim3 gr
     const bool one_wave = (long long)grid.x * grid.y * grid.z <= g_num_sms;
     // wide batch tiles (UMMA N = 256) are throughput-bound per CTA: give them the deepest ring as well
     const int stages = (one_wave || NB == 256) ? C::MAXSTAGES : C::STAGES;
+    // (asking for MORE shared memory than the ring needs, so that PDL successors cannot become co-resident, helps the attention
+    // kernel -- attention.cu -- and changes nothing here: 18 758 / 18 779 / 18 776 tokens/s for +0 / 116 / 160 KB.)
     const int smem = C::smem_bytes(stages, EPI == EPI_QKV);
     TcDev d2 = d; d2.stages = stages;
     {   // per launch: a per-process flag would miss a second device
@@ -552,7 +551,6 @@ int tc_plan(int N, int K, int m_max, bool swiglu, bool has_scratch, int* kb_per_
 int launch_linear_tc(const TcLinearArgs& t, cudaStream_t st) {
     if (t.m_max <= 0) return 0;
     TcDev d;
-    d.pf = t.pf;
     d.K = t.K; d.N = t.N; d.n_kb = t.K / TC_BK; d.m_dev = t.m_dev; d.m_max = t.m_max; d.Y = t.Y; d.ldy = t.ldy; d.R = t.R;
     d.xs_out = t.xs_out; d.ld_xs = t.ld_xs; d.norm_next = t.norm_next; d.ssq_out = t.ssq_out; d.ssq_in = t.ssq_in;
     d.ssq_in_tiles = t.ssq_in_tiles; d.ssq_ld = t.ssq_ld; d.eps = t.eps; d.k_norm = t.k_norm; d.scratch = t.scratch;

@@ -4,7 +4,6 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
-#include "kernels.cuh"
 
 namespace sagc {
 
@@ -79,25 +78,6 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, float (&v)[32]) {
     asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
 #pragma unroll
     for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
-}
-
-// L2 prefetch of the NEXT GEMM's weights, issued by the current kernel once its own loads are out: weights never
-// depend on activations, so the bus that would idle through this kernel's epilogue and the next kernel's prologue
-// brings the leading k blocks of every weight stream of the next kernel into L2.
-__device__ __forceinline__ void tc_prefetch_next(const TcPf& pf, int cta, int n_cta) {
-    if (pf.maps == nullptr || pf.nkb <= 0) return;
-    const int streams = (pf.tiles[0] + pf.tiles[1] + pf.tiles[2]) * pf.ks;
-    const int total = streams * pf.nkb;
-    for (int i = cta; i < total; i += n_cta) {
-        const int j = i / streams, sidx = i - j * streams;       // block j of every stream before block j + 1 of any
-        int t = sidx / pf.ks;
-        const int r = sidx - t * pf.ks;
-        int m = 0;
-        while (m < pf.n_maps - 1 && t >= pf.tiles[m]) { t -= pf.tiles[m]; ++m; }
-        const CUtensorMap* map = reinterpret_cast<const CUtensorMap*>(pf.maps) + m;
-        asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];\n" ::"l"(map), "r"((r * pf.kbpc + j) * 64), "r"(t * 128)
-                     : "memory");
-    }
 }
 
 // K-major, 128-byte-swizzled operand tile (rows of 64 bf16 = 128 B, 8-row atoms of 1024 B):
