@@ -254,6 +254,7 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
             const uint32_t q_a = smem_u32(q_s), p_a = smem_u32(p_s);
             mbar_wait(&sm->q_ready, 0);
             tc_fence_after();
+            const uint64_t dq0 = umma_desc_sw128(q_a);
             // Two independent queues served by whichever is ready (a blocking wait on one would hold the other up and,
             // through the K/V ring, starve itself): S of tile is (needs its K/V tile and a free S buffer: S of tile
             // is - 4 has been consumed once p_full of that tile was seen), P.V of tile ip (needs that tile's P).
@@ -265,14 +266,15 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
                     if (__any_sync(0xffffffffu, mbar_test(&sm->kv_full[s], (uint32_t)((is / NS) & 1)))) {
                         if (lane == 0) ATC_MARK(1, is, 1);
                         tc_fence_after();
-                        const uint32_t k_a = smem_u32(smem + (size_t)s * C::KV_BYTES + (size_t)C::HALVES * C::HALF_BYTES);
+                        // one descriptor per operand tile; a k step only advances the start-address field (bytes >> 4), which
+                        // cannot carry out of its 14 bits here (every tile lies inside the 227 KB window, 16-byte aligned)
+                        const uint64_t da0 = umma_desc_sw128(smem_u32(smem + (size_t)s * C::KV_BYTES + (size_t)C::HALVES * C::HALF_BYTES));
                         const int sb = 2 * (is & 1) + ((is >> 1) & 1);
+                        const uint32_t d_s = tmem_base + 16 * sb;
 #pragma unroll
-                        for (int ks = 0; ks < HD / 16; ++ks) {
-                            const uint64_t da = umma_desc_sw128(k_a + (ks >> 2) * C::HALF_BYTES + (ks & 3) * 32);
-                            const uint64_t db = umma_desc_sw128(q_a + (ks >> 2) * 2048 + (ks & 3) * 32);
-                            tc_mma_e(tmem_base + 16 * sb, da, db, idesc_s, ks > 0 ? 1u : 0u);
-                        }
+                        for (int ks = 0; ks < HD / 16; ++ks)
+                            tc_mma_e(d_s, da0 + (uint64_t)(((ks >> 2) * C::HALF_BYTES + (ks & 3) * 32) >> 4),
+                                     dq0 + (uint64_t)(((ks >> 2) * 2048 + (ks & 3) * 32) >> 4), idesc_s, ks > 0 ? 1u : 0u);
                         tc_commit_e(&sm->s_full[sb]);
                         if (lane == 0) ATC_MARK(1, is, 2);
                         ++is;
@@ -284,13 +286,13 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
                     if (__any_sync(0xffffffffu, mbar_test(&sm->p_full[pb], (uint32_t)((j >> 1) & 1)))) {
                         if (lane == 0) ATC_MARK(1, ip, 3);
                         tc_fence_after();
-                        const uint32_t v_a = smem_u32(smem + (size_t)s * C::KV_BYTES);
+                        const uint64_t dv0 = umma_desc_mn_sw128(smem_u32(smem + (size_t)s * C::KV_BYTES), C::HALF_BYTES);
+                        const uint64_t dp0 = umma_desc_sw128(p_a + pb * C::P_BYTES);
+                        const uint32_t d_o = tmem_base + 64 + 16 * g;
 #pragma unroll
-                        for (int ks = 0; ks < ATC_TILE / 16; ++ks) {
-                            const uint64_t da = umma_desc_mn_sw128(v_a + ks * 2048, C::HALF_BYTES);
-                            const uint64_t db = umma_desc_sw128(p_a + pb * C::P_BYTES + (ks >> 2) * 2048 + (ks & 3) * 32);
-                            tc_mma_e(tmem_base + 64 + 16 * g, da, db, idesc_o, (j > 0 || ks > 0) ? 1u : 0u);
-                        }
+                        for (int ks = 0; ks < ATC_TILE / 16; ++ks)
+                            tc_mma_e(d_o, dv0 + (uint64_t)((ks * 2048) >> 4), dp0 + (uint64_t)(((ks >> 2) * 2048 + (ks & 3) * 32) >> 4), idesc_o,
+                                     (j > 0 || ks > 0) ? 1u : 0u);
                         tc_commit_e(&sm->kv_empty[s]);
                         tc_commit_e(&sm->p_free[pb]);
                         if (lane == 0) ATC_MARK(1, ip, 4);

@@ -536,7 +536,7 @@ static int round_bucket(int live) {
 }
 
 static constexpr int ATT_TC_FLAG = 0x1000;      // pick_splits: this step's attention runs on the tcgen05 kernel
-static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
+static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound, int live) {
     const int ctas = m_bucket * m->cfg.n_kv_heads;
     const int target = (3 * sagc::g_num_sms) / 2;
     int want = target / ctas;                  // ~1.5 CTAs per SM; no split once the grid fills the chip
@@ -553,16 +553,18 @@ static int pick_splits(const sagc_model* m, int m_bucket, int ctx_bound) {
     // the time: it wins from ~2 000 cached tokens per row, or at any context once the grid is large (256 rows x 1 100 tokens:
     // 104 vs 159 us); with few rows at ~1 000 tokens it loses (19.5 vs 17.1 us).  The choice travels in bit 12 of the split count.
     if (m->att_tc && m->cfg.head_dim >= 64 && (m_bucket >= 32 || ctx_bound >= 2048 || m->att_tc > 1)) {
-        // tcgen05 decode attention: one CTA per SM (the K/V ring fills shared memory), >= 2 tiles of 128 tokens per
-        // split, partials merged through L2 by the last arriver; more than 16 splits cost more in the merge than they
-        // save in the scan (1 row x 16 000 tokens: 26 us with 16 splits, 30 us with 32)
-        int w2 = sagc::g_num_sms / ctas;
+        // tcgen05 decode attention: one CTA per SM (the K/V ring fills shared memory), >= 2 tiles of 128 tokens per split,
+        // partials merged through L2 by the last arriver, so ANY split count works: it is sized by the rows that are really
+        // live (exact with forced lengths, a polled upper bound otherwise), not by the batch bucket -- in the 7B tail the
+        // bucket of 8 holds 4.2 rows on average and attention is 25 % of the step (SAGC_SKIP ablation).  More than 16 splits
+        // cost more in the merge than they save in the scan (1 row x 16 000 tokens: 26 us with 16 splits, 30 us with 32).
+        const int rows = live > 0 && live < m_bucket ? live : m_bucket;
+        int w2 = sagc::g_num_sms / (rows * m->cfg.n_kv_heads);
         const int cap2 = ctx_bound / 256;
         if (w2 > cap2) w2 = cap2;
         if (w2 > 16) w2 = 16;
         if (w2 > m->max_splits) w2 = m->max_splits;
-        s = 1;
-        while (s * 2 <= w2) s *= 2;
+        s = w2 < 1 ? 1 : w2;
         s |= ATT_TC_FLAG;
     }
     return s;
@@ -888,7 +890,7 @@ extern "C" int sagc_rollout_group(sagc_model* m, const int32_t* prompt_tokens, c
             const int mb = round_bucket(live);
             const int kind = pick_kind(m, prm->path, mb);
             const bool mega = step_kernel_applies(m, kind, mb);
-            const int ns = mega ? 0 : pick_splits(m, mb, pmax + t - 1);      // the step kernel picks its K-splits on the device
+            const int ns = mega ? 0 : pick_splits(m, mb, pmax + t - 1, live);      // the step kernel picks its K-splits on the device
             if (mega && !prev_mega)       // both counter sets must be clear when the step kernel takes over
                 CU(cudaMemsetAsync(m->step_sync, 0, (size_t)2 * (m->gbar_n + m->tcnt_n) * sizeof(unsigned), st));
             prev_mega = mega;
