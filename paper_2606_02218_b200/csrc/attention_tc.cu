@@ -193,6 +193,7 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
         for (int b = 0; b < 4; ++b) { mbar_init(&sm->s_full[b], 1); mbar_init(&sm->p_full[b], 4); mbar_init(&sm->p_free[b], 1); }
         mbar_init(&sm->q_ready, 4); mbar_init(&sm->app_done, 4); mbar_init(&sm->o_done, 1);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        sm->last_s = 0;
         tma_prefetch_desc(&kvmap);
     }
     if (warp == 1) {
@@ -480,10 +481,10 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
 #pragma unroll
         for (int h = 0; h < 8; ++h) l[h] = (sm->l_s[wg][0][h] + sm->l_s[wg][1][h]) + (sm->l_s[wg][2][h] + sm->l_s[wg][3][h]);
         // ---- the odd tiles' (o, m, l) join the even tiles' (same log-sum-exp rule as the split merge) ----
-        float* xo = reinterpret_cast<float*>(p_s);          // [d][8], overlays the P buffers
+        float* xo = reinterpret_cast<float*>(p_s);          // [8][128 d] (conflict-free for thread = d), overlays the P buffers
         if (wg == 1) {
 #pragma unroll
-            for (int h = 0; h < 8; h += 4) *reinterpret_cast<float4*>(xo + tl * 8 + h) = make_float4(ov[h], ov[h + 1], ov[h + 2], ov[h + 3]);
+            for (int h = 0; h < 8; ++h) xo[h * 128 + tl] = ov[h];
             if (st == 0) {
 #pragma unroll
                 for (int h = 0; h < 8; ++h) { sm->xm[h] = m_used[h]; sm->xl[h] = l[h]; }
@@ -498,7 +499,7 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
             const float mb = sm->xm[h], mn = fmaxf(m_used[h], mb);
             const float fa = (m_used[h] == -INFINITY) ? 0.f : __expf(m_used[h] - mn);
             const float fb = (mb == -INFINITY) ? 0.f : __expf(mb - mn);
-            ov[h] = ov[h] * fa + xo[tl * 8 + h] * fb;
+            ov[h] = ov[h] * fa + xo[h * 128 + tl] * fb;
             l[h] = l[h] * fa + sm->xl[h] * fb;
             m_used[h] = mn;
         }
@@ -531,60 +532,59 @@ __global__ void __launch_bounds__(ATC_THREADS, 1) k_attention_tc(const __grid_co
             }
             bar_softmax(0);
             if (st == 0) ATC_MARK(2, 62, 5);
-            if (sm->last_s) {
-                // ---- merge: this unit arrived last for (row, kv head); arithmetic of attention_body.cuh ----
-                __threadfence();
-                for (int h = sw; h < r; h += 4) {
-                    const float* ml = a.part_ml + ((size_t)row * a.Hq + kvh * r + h) * nsp * 2;
-                    float mv[2], lv[2];
-#pragma unroll
-                    for (int u = 0; u < 2; ++u) {
-                        const int s2 = lane + 32 * u;
-                        mv[u] = (s2 < nsp) ? __ldcg(ml + 2 * s2) : -INFINITY;
-                        lv[u] = (s2 < nsp) ? __ldcg(ml + 2 * s2 + 1) : 0.f;
-                    }
-                    const float mx = warp_max(fmaxf(mv[0], mv[1]));
-                    float f[2];
-#pragma unroll
-                    for (int u = 0; u < 2; ++u) f[u] = (lv[u] > 0.f) ? __expf(mv[u] - mx) : 0.f;
-                    const float den = warp_sum(f[0] * lv[0] + f[1] * lv[1]);
-#pragma unroll
-                    for (int u = 0; u < 2; ++u)
-                        if (lane + 32 * u < nsp) sm->wgt[h * nsp + lane + 32 * u] = f[u] / den;
-                }
-                bar_softmax(0);
-                // every thread combines r * HD / 128 outputs; the loads of 8 splits x 2 outputs are in flight together
-                // (the partials sit in L2: the merge is a chain of round trips, not bandwidth)
-                const int n_out = r * HD;
-                for (int i0 = st; i0 < n_out; i0 += 256) {
-                    const int i1 = i0 + 128;
-                    const bool two = i1 < n_out;
-                    const int h0 = i0 / HD, d0 = i0 % HD, h1 = two ? i1 / HD : h0, d1 = two ? i1 % HD : d0;
-                    const float* po0 = a.part_o + ((size_t)row * a.Hq + kvh * r + h0) * nsp * HD + d0;
-                    const float* po1 = a.part_o + ((size_t)row * a.Hq + kvh * r + h1) * nsp * HD + d1;
-                    const float* w0 = sm->wgt + h0 * nsp;
-                    const float* w1 = sm->wgt + h1 * nsp;
-                    float n0 = 0.f, n1 = 0.f;
-                    for (int s0 = 0; s0 < nsp; s0 += 8) {
-                        float v0[8], v1[8];
-#pragma unroll
-                        for (int u = 0; u < 8; ++u) {
-                            const int s2 = min(s0 + u, nsp - 1);
-                            v0[u] = __ldcg(po0 + (size_t)s2 * HD);
-                            v1[u] = __ldcg(po1 + (size_t)s2 * HD);
-                        }
-#pragma unroll
-                        for (int u = 0; u < 8; ++u)
-                            if (s0 + u < nsp) { n0 += w0[s0 + u] * v0[u]; n1 += w1[s0 + u] * v1[u]; }
-                    }
-                    store_out(a, row, (kvh * r + h0) * HD + d0, n0);
-                    if (two) store_out(a, row, (kvh * r + h1) * HD + d1, n1);
-                }
-                if (st == 0) ATC_MARK(2, 62, 6);
-                if (st == 0) a.counters[row * a.Hkv + kvh] = 0;
-            }
         }
         }   // warpgroup 0
+    }
+    // ---- merge by the unit that arrived last for (row, kv head): ALL 320 threads (the partials sit in L2, so the merge is a
+    // chain of round trips: the more loads in flight the shorter); arithmetic of attention_body.cuh ----
+    if (nsp > 1) __syncthreads();            // (nsp is uniform over the CTA; the unsplit path has nothing to merge)
+    if (nsp > 1 && sm->last_s) {
+        __threadfence();
+        for (int h = warp; h < r; h += ATC_THREADS / 32) {
+            const float* ml = a.part_ml + ((size_t)row * a.Hq + kvh * r + h) * nsp * 2;
+            float mv[2], lv[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int s2 = lane + 32 * u;
+                mv[u] = (s2 < nsp) ? __ldcg(ml + 2 * s2) : -INFINITY;
+                lv[u] = (s2 < nsp) ? __ldcg(ml + 2 * s2 + 1) : 0.f;
+            }
+            const float mx = warp_max(fmaxf(mv[0], mv[1]));
+            float f[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) f[u] = (lv[u] > 0.f) ? __expf(mv[u] - mx) : 0.f;
+            const float den = warp_sum(f[0] * lv[0] + f[1] * lv[1]);
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+                if (lane + 32 * u < nsp) sm->wgt[h * nsp + lane + 32 * u] = f[u] / den;
+        }
+        __syncthreads();
+        const int n_out = r * HD;
+        for (int i0 = tid; i0 < n_out; i0 += 2 * ATC_THREADS) {      // two outputs x 8 splits in flight per thread
+            const int i1 = i0 + ATC_THREADS;
+            const bool two = i1 < n_out;
+            const int h0 = i0 / HD, d0 = i0 % HD, h1 = two ? i1 / HD : h0, d1 = two ? i1 % HD : d0;
+            const float* po0 = a.part_o + ((size_t)row * a.Hq + kvh * r + h0) * nsp * HD + d0;
+            const float* po1 = a.part_o + ((size_t)row * a.Hq + kvh * r + h1) * nsp * HD + d1;
+            const float* w0 = sm->wgt + h0 * nsp;
+            const float* w1 = sm->wgt + h1 * nsp;
+            float n0 = 0.f, n1 = 0.f;
+            for (int s0 = 0; s0 < nsp; s0 += 8) {
+                float v0[8], v1[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const int s2 = min(s0 + u, nsp - 1);
+                    v0[u] = __ldcg(po0 + (size_t)s2 * HD);
+                    v1[u] = __ldcg(po1 + (size_t)s2 * HD);
+                }
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+                    if (s0 + u < nsp) { n0 += w0[s0 + u] * v0[u]; n1 += w1[s0 + u] * v1[u]; }
+            }
+            store_out(a, row, (kvh * r + h0) * HD + d0, n0);
+            if (two) store_out(a, row, (kvh * r + h1) * HD + d1, n1);
+        }
+        if (tid == 0) { ATC_MARK(2, 62, 6); a.counters[row * a.Hkv + kvh] = 0; }
     }
     tc_fence_before();
     __syncthreads();
