@@ -1,5 +1,5 @@
 // attention_tc.cu -- paged GQA decode attention (step a7) on the 5th-generation tensor cores: the decode-step
-// attention of head_dim 64 / 128 models.  One CTA per (activation row, kv head, K-split), 192 threads:
+// attention of head_dim 64 / 128 models.  One CTA per (activation row, kv head, K-split), 320 threads:
 //
 //   warp 0     TMA producer: per 128-token tile, one cp.async.bulk.tensor box per (page, K|V, 64-wide half of the
 //              head) of the paged pool -- the pool of a layer is a 2-D tensor [n_pages * 2 * Hkv * page][hd], so a
@@ -9,7 +9,8 @@
 //                O^T[d][n]    += V[token][d] . P[n][token]     A = V tile (MN-major: the tile IS V^T for the MMA),
 //                                                              B = P (16 rows: heads hi | lo, K-major over tokens)
 //              S of tile i+1 is issued before P.V of tile i, so the softmax of a tile overlaps both neighbours.
-//   warps 2-5  softmax: thread = token (TMEM lane).  It reads its 16 S columns (tcgen05.ld), adds the hi and lo
+//   warps 2-9  two softmax warpgroups on alternate tiles (own S / P buffers and O accumulator, joined at the end by the
+//              log-sum-exp rule): thread = token (TMEM lane).  It reads its 16 S columns (tcgen05.ld), adds the hi and lo
 //              column of each head, takes the tile maximum per head over the 128 tokens (redux.sync on order-preserving
 //              integers + one 128-thread named barrier), exponentiates, accumulates its share of the row sums and
 //              writes p as bf16 hi + lo into the swizzled P operand.  The running maximum is LAZY: it moves (and O in
@@ -18,7 +19,7 @@
 //
 // Precision is the register-HMMA unit's (attention_body.cuh): K, V exact bf16; q and p as hi + lo bf16 pairs
 // (~16 mantissa bits); fp32 accumulation.  Split-K partials (o, m, l) merge through the L2 scratch by the last unit
-// to arrive, with the arithmetic of attention_body.cuh.  Decode (fuse_rope): RoPE of q / k and the bf16 K,V append
+// to arrive (all 320 threads of that CTA), with the arithmetic of attention_body.cuh.  Decode (fuse_rope): RoPE of q / k and the bf16 K,V append
 // of the newest position happen here; the split that owns that position appends BEFORE its producer fetches the
 // last tile (generic -> async proxy fence + mbarrier), so no shared-memory patching is needed.
 // Masked positions: p = 0 exactly, and the pool is finite everywhere (zeroed at creation), so stale V rows of a
