@@ -178,7 +178,7 @@ def _attention_case(rng, ctxs, Hq, Hkv, hd, page):
     return q, kv, pt, ref
 
 
-@pytest.mark.parametrize("Hq,Hkv,hd,page", [(4, 4, 32, 16), (14, 2, 64, 64), (28, 4, 128, 64), (8, 1, 128, 32)])
+@pytest.mark.parametrize("Hq,Hkv,hd,page", [(4, 4, 32, 16), (14, 2, 64, 64), (28, 4, 128, 64), (8, 1, 128, 32), (8, 2, 64, 16), (12, 2, 128, 128)])
 @pytest.mark.parametrize("splits,variant", [(1, 0), (2, 0), (4, 0), (8, 0), (16, 0), (1, 1), (3, 1), (8, 1), (32, 1),
                                             (1, 2), (2, 2), (5, 2), (12, 2), (64, 2)])
 def test_paged_attention_vs_fp64(B, Hq, Hkv, hd, page, splits, variant):
